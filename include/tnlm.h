@@ -1,0 +1,155 @@
+/*
+ * tnlm.h -- C ABI of libtnlm.so: the temporal non-local means (TNLM) enhancement hot path of
+ * arxiv/paper_1201_2450 (Jia, Tian, Lou, Sonke, Jiang) as hand-written sm_100a CUDA kernels.
+ *
+ * Citations are lines of the paper text with the equation they fall in.
+ *
+ * Data model: a 4D image stack {f_i}, i = 1..N_p respiratory phases,
+ * cyclic in i (f_{N_p+1} = f_1), stored as ONE contiguous fp32 array [n_phase][nz][ny][nx],
+ * x fastest.  All stack pointers below are DEVICE pointers on the current CUDA device unless a
+ * function name ends in _host.  They are allocated and freed by the caller, must be 16-byte
+ * aligned, and are only read or written by work enqueued on `cuda_stream` (a cudaStream_t passed
+ * as void*; NULL = the legacy default stream).  Calls enqueue and return; results are valid
+ * once the stream has been synchronised.  The library allocates no device memory and keeps no
+ * global state (except the text of the last CUDA error of the calling thread); calls on different
+ * streams with distinct workspaces may run concurrently.
+ *
+ * Boundary handling (the paper is silent; reading P4): every read of a stack at a
+ * coordinate outside the volume returns the nearest in-volume voxel (clamp-to-edge), so every
+ * voxel has its full (2M+1)^3 search window.  Phases are taken mod n_phase.
+ *
+ * Errors: every int-returning function returns TNLM_OK (0) or a negative tnlm_status.  Argument
+ * errors are detected synchronously, before anything is enqueued; on error no output is written.
+ * NaN/Inf in the inputs are not scanned for (they propagate).  No C++ exception crosses the ABI.
+ */
+#ifndef TNLM_H_
+#define TNLM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+    int32_t n_phase, nz, ny, nx; /* stack [n_phase][nz][ny][nx], fp32, contiguous; n_phase >= 2   */
+    int32_t patch_radius;        /* d >= 0: patch = (2d+1)^3 cube centred at the voxel */
+    int32_t search_radius;       /* M >= 0: search window (2M+1)^3 centred at x       */
+    float h;                     /* > 0, finite: similarity scale of Eq. 3            */
+    float mu;                    /* > 0, finite: fidelity weight of Eq. 4             */
+} tnlm_params;
+
+typedef enum {
+    TNLM_OK = 0,
+    TNLM_ERR_NULL_POINTER = -1, /* a required pointer is NULL                                      */
+    TNLM_ERR_BAD_DIMS = -2,     /* an extent < 1, n_phase < 2 (a phase is never compared with
+                                   itself), or the stack exceeds 2^31-1 voxels       */
+    TNLM_ERR_BAD_PARAM = -3,    /* h or mu not finite or <= 0; negative radius; n_iter < 0         */
+    TNLM_ERR_UNSUPPORTED = -4,  /* radius outside the compiled set (d <= 3, M <= 6), bad variant   */
+    TNLM_ERR_ALIAS = -5,        /* f_out overlaps an input (Jacobi reads only the old iterate,
+                                   PAPER.md:176) or the workspace                                  */
+    TNLM_ERR_WORKSPACE = -6,    /* workspace NULL, too small or not 16-byte aligned                */
+    TNLM_ERR_CUDA = -7          /* a CUDA call failed; tnlm_strerror(TNLM_ERR_CUDA) has the text   */
+} tnlm_status;
+
+/* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M). */
+enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2 };
+
+/*
+ * Bytes of caller-owned device workspace that tnlm_jacobi_step / tnlm_enhance / tnlm_weights need
+ * for these parameters (the second iterate buffer of the Jacobi double buffering plus kernel
+ * scratch).  Returns 0 if the parameters are invalid.
+ */
+size_t tnlm_workspace_bytes(const tnlm_params *p);
+
+/* Bytes of the w_out array of tnlm_weights: n_phase*2*(2M+1)^3*nz*ny*nx*4; 0 if invalid or overflow. */
+size_t tnlm_weights_bytes(const tnlm_params *p);
+
+/*
+ * Normalised TNLM weights of Eq. 3 estimated from `ref` as in Eq. 9:
+ *   w_out[p][s][k][z][y][x] = exp(-D_k(x)/2h^2) / sum_k' exp(-D_k'(x)/2h^2),
+ *   D_k(x) = sum_{delta in [-d,d]^3} (ref_p(x+delta) - ref_q(x+t_k+delta))^2   (plain l2),
+ *   q = p-1 for s = 0, q = p+1 for s = 1 (cyclic); t_k = (tz,ty,tx) in [-M,M]^3 with
+ *   k = ((tz+M)(2M+1) + (ty+M))(2M+1) + (tx+M); the candidate voxel is y = x + t_k.
+ * The normaliser runs over the candidates of ONE voxel x and ONE neighbour phase (PAPER.md:105 with
+ * the coefficients of Eq. 7), so sum_k w = 1 for every (p, s, x).  The exponentials
+ * are evaluated relative to the smallest D of the window (identical to Eq. 3, never 0/0).
+ * For inspection and tests: config 3 of BASELINE.json would need 84 GB.  ws may be NULL.
+ */
+int tnlm_weights(const tnlm_params *p, const float *ref, float *w_out, void *ws, size_t ws_bytes,
+                 void *cuda_stream);
+
+/*
+ * One Gauss-Jacobi sweep of Eq. 8 for all phases, weights of Eq. 9 computed on the
+ * fly from `ref` (never stored):
+ *   f_out_i(x) = mu/(2+mu) g_i(x) + 1/(2+mu) [ sum_y f_{i+1}(y) w_{i,i+1}(x,y) + sum_y f_{i-1}(y) w_{i,i-1}(x,y) ].
+ * ref == NULL means ref = f (TNLM-E); TNLM-R passes ref = g^(k).
+ * All phases read only `f` (pure Jacobi): f_out must not overlap f, g, ref or ws.
+ * n_phase == 2 is legal: phases i+1 and i-1 coincide and are counted twice, as Eq. 8 reads.
+ */
+int tnlm_jacobi_step(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out,
+                     void *ws, size_t ws_bytes, void *cuda_stream);
+
+/* Same, with an explicit kernel variant (TNLM_VARIANT_*); TNLM_ERR_UNSUPPORTED if that variant is
+ * not compiled for (d, M). */
+int tnlm_jacobi_step_variant(const tnlm_params *p, const float *f, const float *g, const float *ref,
+                             float *f_out, void *ws, size_t ws_bytes, void *cuda_stream, int variant);
+
+/*
+ * TNLM enhancement, TNLM-E: f^0 = f_init (NULL => g); n_iter times
+ * { weights from f^k (Eq. 9); one sweep of Eq. 8 }.  A fixed iteration count replaces "until
+ * convergence" (the paper ran 10).  No positivity clamp (that is TNLM-R step 4 only,
+ * PAPER.md:200).  n_iter == 0 copies f^0 to f_out.  f_out must not overlap g, f_init or ws.
+ * To resume, pass the earlier result as f_init together with the ORIGINAL g.
+ */
+int tnlm_enhance(const tnlm_params *p, const float *g, const float *f_init, float *f_out, int32_t n_iter,
+                 void *ws, size_t ws_bytes, void *cuda_stream);
+
+int tnlm_enhance_variant(const tnlm_params *p, const float *g, const float *f_init, float *f_out,
+                         int32_t n_iter, void *ws, size_t ws_bytes, void *cuda_stream, int variant);
+
+/*
+ * End-to-end form of tnlm_enhance for HOST buffers: g_host / f_init_host (may be NULL) / f_out_host
+ * are host pointers (pinned memory makes the copies asynchronous).  The call copies the inputs to the
+ * device, runs tnlm_enhance and copies the result back, all on `cuda_stream`, then synchronises the
+ * stream before returning.  dev_ws is a caller-owned DEVICE workspace of at least
+ * tnlm_host_workspace_bytes(p) bytes (it holds the device stacks as well as the kernel workspace).
+ */
+size_t tnlm_host_workspace_bytes(const tnlm_params *p);
+int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
+                      int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream);
+
+/*
+ * Z-slab form of one sweep for data-parallel sharding: computes only the
+ * output planes z in [z_begin, z_end) of every phase.  f, g, ref and f_out are FULL stacks (the rank
+ * needs planes within M+d of its slab to be valid in f / ref); planes outside the slab are untouched.
+ */
+int tnlm_jacobi_step_slab(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out,
+                          int32_t z_begin, int32_t z_end, void *ws, size_t ws_bytes, void *cuda_stream);
+
+int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const float *g, const float *ref,
+                                  float *f_out, int32_t z_begin, int32_t z_end, void *ws, size_t ws_bytes,
+                                  void *cuda_stream, int variant);
+
+/* Message for a status code; for TNLM_ERR_CUDA includes the calling thread's last CUDA error text. */
+const char *tnlm_strerror(int code);
+
+/* Name of the kernel that TNLM_VARIANT_AUTO selects for these parameters (static string). */
+const char *tnlm_kernel_name(const tnlm_params *p);
+
+/* Number of kernel launches one tnlm_jacobi_step enqueues for these parameters (>= 1), 0 if invalid. */
+int32_t tnlm_launches_per_sweep(const tnlm_params *p);
+
+/*
+ * Measurement aid for the FP32 roofline: enqueues a register-resident FFMA
+ * loop on every SM; it executes exactly tnlm_probe_fp32_ffma_count(n_iter) FFMA lane-operations.
+ * sink is a device buffer of at least 4 bytes.  Time it with CUDA events on `cuda_stream`.
+ */
+int tnlm_probe_fp32(int32_t n_iter, float *sink, void *cuda_stream);
+double tnlm_probe_fp32_ffma_count(int32_t n_iter);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TNLM_H_ */

@@ -1,0 +1,211 @@
+"""ctypes binding of libtnlm.so: same names as include/tnlm.h, argument marshalling only.
+
+Stacks are torch CUDA tensors of dtype float32 and shape [n_phase][nz][ny][nx] (contiguous);
+PyTorch provides device memory and streams, nothing else.  Every function raises TnlmError with
+the library's message on a non-zero status.  The library must have been built
+(``python -m paper_1201_2450_b200._build`` or ``__graft_entry__.build()``); a missing library is
+an error, never a fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED = 0, 1, 2
+
+# every symbol include/tnlm.h declares
+EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_jacobi_step",
+           "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
+           "tnlm_enhance_host", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
+           "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count"]
+
+
+class TnlmParams(C.Structure):
+    """Mirror of ``tnlm_params`` (include/tnlm.h)."""
+    _fields_ = [("n_phase", C.c_int32), ("nz", C.c_int32), ("ny", C.c_int32), ("nx", C.c_int32),
+                ("patch_radius", C.c_int32), ("search_radius", C.c_int32), ("h", C.c_float), ("mu", C.c_float)]
+
+    @classmethod
+    def make(cls, shape, patch_radius, search_radius, h, mu):
+        P, Z, Y, X = (int(v) for v in shape)
+        return cls(P, Z, Y, X, int(patch_radius), int(search_radius), float(h), float(mu))
+
+    @property
+    def shape(self):
+        return (self.n_phase, self.nz, self.ny, self.nx)
+
+
+class TnlmError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = int(code)
+        super().__init__(f"{what}: tnlm status {code}: {strerror(code)}")
+
+
+_LIB = None
+
+
+def library_path() -> str:
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libtnlm.so")
+
+
+def lib():
+    global _LIB
+    if _LIB is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: build it with `python -m paper_1201_2450_b200._build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        pp, vp, i32, sz = C.POINTER(TnlmParams), C.c_void_p, C.c_int32, C.c_size_t
+        L.tnlm_workspace_bytes.argtypes = [pp]; L.tnlm_workspace_bytes.restype = sz
+        L.tnlm_weights_bytes.argtypes = [pp]; L.tnlm_weights_bytes.restype = sz
+        L.tnlm_host_workspace_bytes.argtypes = [pp]; L.tnlm_host_workspace_bytes.restype = sz
+        L.tnlm_weights.argtypes = [pp, vp, vp, vp, sz, vp]
+        L.tnlm_jacobi_step.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp]
+        L.tnlm_jacobi_step_variant.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp, C.c_int]
+        L.tnlm_jacobi_step_slab.argtypes = [pp, vp, vp, vp, vp, i32, i32, vp, sz, vp]
+        L.tnlm_jacobi_step_slab_variant.argtypes = [pp, vp, vp, vp, vp, i32, i32, vp, sz, vp, C.c_int]
+        L.tnlm_enhance.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp]
+        L.tnlm_enhance_variant.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp, C.c_int]
+        L.tnlm_enhance_host.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp]
+        L.tnlm_strerror.argtypes = [C.c_int]; L.tnlm_strerror.restype = C.c_char_p
+        L.tnlm_kernel_name.argtypes = [pp]; L.tnlm_kernel_name.restype = C.c_char_p
+        L.tnlm_launches_per_sweep.argtypes = [pp]; L.tnlm_launches_per_sweep.restype = i32
+        L.tnlm_probe_fp32.argtypes = [i32, vp, vp]
+        L.tnlm_probe_fp32_ffma_count.argtypes = [i32]; L.tnlm_probe_fp32_ffma_count.restype = C.c_double
+        _LIB = L
+    return _LIB
+
+
+def strerror(code) -> str:
+    return lib().tnlm_strerror(int(code)).decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise TnlmError(rc, what)
+
+
+def workspace_bytes(p: TnlmParams) -> int:
+    return int(lib().tnlm_workspace_bytes(C.byref(p)))
+
+
+def weights_bytes(p: TnlmParams) -> int:
+    return int(lib().tnlm_weights_bytes(C.byref(p)))
+
+
+def host_workspace_bytes(p: TnlmParams) -> int:
+    return int(lib().tnlm_host_workspace_bytes(C.byref(p)))
+
+
+def kernel_name(p: TnlmParams) -> str:
+    return lib().tnlm_kernel_name(C.byref(p)).decode()
+
+
+def launches_per_sweep(p: TnlmParams) -> int:
+    return int(lib().tnlm_launches_per_sweep(C.byref(p)))
+
+
+# ---- torch marshalling ------------------------------------------------------------------------
+def _dev_ptr(t, p: TnlmParams, name, optional=False):
+    if t is None:
+        if optional:
+            return None
+        raise TnlmError(-1, f"{name} is None")
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA torch tensor (no CPU path exists)")
+    if t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != p.shape:
+        raise TypeError(f"{name} must be contiguous float32 of shape {p.shape}, got {t.dtype} {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def _workspace(p: TnlmParams, ws, nbytes=None):
+    import torch
+    need = workspace_bytes(p) if nbytes is None else nbytes
+    if ws is None:
+        ws = torch.empty(max(need, 16), dtype=torch.uint8, device="cuda")
+    if not ws.is_cuda or ws.dtype != torch.uint8:
+        raise TypeError("workspace must be a CUDA uint8 tensor")
+    return ws
+
+
+def tnlm_weights(p: TnlmParams, ref, w_out=None, stream=None):
+    """Normalised weights w[p][s][k][z][y][x] of Eq. 3/9 (see include/tnlm.h)."""
+    import torch
+    n_t = (2 * p.search_radius + 1) ** 3
+    if w_out is None:
+        w_out = torch.empty((p.n_phase, 2, n_t, p.nz, p.ny, p.nx), dtype=torch.float32, device=ref.device)
+    _check(lib().tnlm_weights(C.byref(p), _dev_ptr(ref, p, "ref"), w_out.data_ptr(), None, 0, _stream(stream)),
+           "tnlm_weights")
+    return w_out
+
+
+def tnlm_jacobi_step(p: TnlmParams, f, g, ref=None, f_out=None, ws=None, stream=None, variant=VARIANT_AUTO):
+    """One Gauss-Jacobi sweep of Eq. 8 (see include/tnlm.h)."""
+    import torch
+    if f_out is None:
+        f_out = torch.empty_like(f)
+    ws = _workspace(p, ws)
+    _check(lib().tnlm_jacobi_step_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
+                                          _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
+                                          ws.data_ptr(), ws.numel(), _stream(stream), int(variant)),
+           "tnlm_jacobi_step")
+    return f_out
+
+
+def tnlm_jacobi_step_slab(p: TnlmParams, f, g, z_begin, z_end, ref=None, f_out=None, ws=None, stream=None,
+                          variant=VARIANT_AUTO):
+    import torch
+    if f_out is None:
+        f_out = torch.empty_like(f)
+    ws = _workspace(p, ws)
+    _check(lib().tnlm_jacobi_step_slab_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
+                                               _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
+                                               int(z_begin), int(z_end), ws.data_ptr(), ws.numel(),
+                                               _stream(stream), int(variant)),
+           "tnlm_jacobi_step_slab")
+    return f_out
+
+
+def tnlm_enhance(p: TnlmParams, g, n_iter, f_init=None, f_out=None, ws=None, stream=None, variant=VARIANT_AUTO):
+    """TNLM-E: n_iter x {weights from f^k; one sweep} (see include/tnlm.h)."""
+    import torch
+    if f_out is None:
+        f_out = torch.empty_like(g)
+    ws = _workspace(p, ws)
+    _check(lib().tnlm_enhance_variant(C.byref(p), _dev_ptr(g, p, "g"), _dev_ptr(f_init, p, "f_init", optional=True),
+                                      _dev_ptr(f_out, p, "f_out"), int(n_iter), ws.data_ptr(), ws.numel(),
+                                      _stream(stream), int(variant)),
+           "tnlm_enhance")
+    return f_out
+
+
+def tnlm_enhance_host(p: TnlmParams, g_host, n_iter, f_out_host=None, f_init_host=None, dev_ws=None, stream=None):
+    """End-to-end form with HOST tensors (pinned for asynchronous copies); returns the host result."""
+    import torch
+    for name, t in (("g_host", g_host), ("f_init_host", f_init_host), ("f_out_host", f_out_host)):
+        if t is not None and (t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous()
+                              or tuple(t.shape) != p.shape):
+            raise TypeError(f"{name} must be a contiguous float32 CPU tensor of shape {p.shape}")
+    if f_out_host is None:
+        f_out_host = torch.empty(p.shape, dtype=torch.float32, pin_memory=True)
+    dev_ws = _workspace(p, dev_ws, host_workspace_bytes(p))
+    _check(lib().tnlm_enhance_host(C.byref(p), g_host.data_ptr(),
+                                   None if f_init_host is None else f_init_host.data_ptr(),
+                                   f_out_host.data_ptr(), int(n_iter), dev_ws.data_ptr(), dev_ws.numel(),
+                                   _stream(stream)),
+           "tnlm_enhance_host")
+    return f_out_host
+
+
+def probe_fp32(n_iter: int, sink, stream=None) -> float:
+    """Enqueue the FFMA probe; returns the number of FFMA lane-operations it executes."""
+    _check(lib().tnlm_probe_fp32(int(n_iter), sink.data_ptr(), _stream(stream)), "tnlm_probe_fp32")
+    return float(lib().tnlm_probe_fp32_ffma_count(int(n_iter)))

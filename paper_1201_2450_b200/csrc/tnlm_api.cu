@@ -1,0 +1,297 @@
+// C-ABI entry points of libtnlm.so (include/tnlm.h): argument validation, workspace carving,
+// kernel selection and launch.  Every step of the hot path runs in the kernels of this library.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "tnlm_common.cuh"
+#include "tnlm_generic.cuh"
+#include "tnlm_tiled.cuh"
+
+namespace {
+
+using namespace tnlm;
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char *where)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return TNLM_ERR_CUDA;
+}
+
+constexpr int kMaxPatchRadius = 3;
+constexpr int kMaxSearchRadius = 6;
+
+int check_params(const tnlm_params *p)
+{
+    if (!p) return TNLM_ERR_NULL_POINTER;
+    if (p->n_phase < 2 || p->nz < 1 || p->ny < 1 || p->nx < 1) return TNLM_ERR_BAD_DIMS;
+    const double n = (double)p->n_phase * p->nz * p->ny * p->nx;
+    if (n > 2147483647.0) return TNLM_ERR_BAD_DIMS;
+    if (p->patch_radius < 0 || p->search_radius < 0) return TNLM_ERR_BAD_PARAM;
+    if (!(p->h > 0.f) || !std::isfinite(p->h) || !(p->mu > 0.f) || !std::isfinite(p->mu)) return TNLM_ERR_BAD_PARAM;
+    if (p->patch_radius > kMaxPatchRadius || p->search_radius > kMaxSearchRadius) return TNLM_ERR_UNSUPPORTED;
+    return TNLM_OK;
+}
+
+size_t stack_bytes(const tnlm_params *p) { return (size_t)p->n_phase * p->nz * p->ny * p->nx * sizeof(float); }
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    if (!a || !b || na == 0 || nb == 0) return false;
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + nb && y < x + na;
+}
+
+bool misaligned(const void *p) { return ((uintptr_t)p & 15u) != 0; }
+
+int sm_count()
+{
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+    return n;
+}
+
+int pick_variant(const tnlm_params *p, int variant)
+{
+    if (variant == TNLM_VARIANT_GENERIC) return TNLM_VARIANT_GENERIC;
+    if (variant == TNLM_VARIANT_TILED) return tiled_supported(*p) ? TNLM_VARIANT_TILED : -1;
+    if (variant == TNLM_VARIANT_AUTO) return tiled_supported(*p) ? TNLM_VARIANT_TILED : TNLM_VARIANT_GENERIC;
+    return -1;
+}
+
+// One sweep over the slab [z0, z1); all pointers already validated.
+int launch_sweep(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out, int z0, int z1,
+                 void *kernel_ws, size_t kernel_ws_bytes, cudaStream_t st, int variant)
+{
+    if (z1 <= z0) return TNLM_OK;
+    const Dims dm = make_dims(*p, z0, z1);
+    if (variant == TNLM_VARIANT_TILED) {
+        cudaError_t e = launch_tiled(*p, dm, f, g, ref, f_out, kernel_ws, kernel_ws_bytes, st);
+        return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "tiled sweep launch");
+    }
+    const size_t total = (size_t)p->n_phase * (z1 - z0) * p->ny * p->nx;
+    size_t blocks = (total + 255) / 256;
+    const size_t cap = (size_t)sm_count() * 64;
+    if (blocks > cap) blocks = cap;
+    jacobi_generic_kernel<<<(unsigned)blocks, 256, 0, st>>>(f, g, ref, f_out, dm);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "generic sweep launch");
+}
+
+int check_ws(const tnlm_params *p, const void *ws, size_t ws_bytes)
+{
+    if (!ws) return TNLM_ERR_WORKSPACE;
+    if (misaligned(ws) || ws_bytes < tnlm_workspace_bytes(p)) return TNLM_ERR_WORKSPACE;
+    return TNLM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t tnlm_workspace_bytes(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return 0;
+    // [second iterate buffer][kernel scratch]
+    return align_up(stack_bytes(p), 256) + align_up(tiled_scratch_bytes(*p), 256);
+}
+
+size_t tnlm_weights_bytes(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return 0;
+    const double e = 2.0 * p->search_radius + 1.0;
+    const double n = (double)p->n_phase * 2.0 * e * e * e * p->nz * p->ny * p->nx * 4.0;
+    if (n > 1.8e19) return 0;
+    return (size_t)n;
+}
+
+size_t tnlm_host_workspace_bytes(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return 0;
+    // [g][f_init][f_out][tnlm_enhance workspace]
+    return 3 * align_up(stack_bytes(p), 256) + tnlm_workspace_bytes(p);
+}
+
+int tnlm_weights(const tnlm_params *p, const float *ref, float *w_out, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    (void)ws; (void)ws_bytes;
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!ref || !w_out) return TNLM_ERR_NULL_POINTER;
+    const size_t wb = tnlm_weights_bytes(p);
+    if (wb == 0) return TNLM_ERR_BAD_DIMS;
+    if (misaligned(ref) || misaligned(w_out)) return TNLM_ERR_WORKSPACE;
+    if (overlaps(w_out, wb, ref, stack_bytes(p))) return TNLM_ERR_ALIAS;
+    const Dims dm = make_dims(*p, 0, p->nz);
+    const size_t total = (size_t)p->n_phase * 2 * p->nz * p->ny * p->nx;
+    size_t blocks = (total + 255) / 256;
+    const size_t cap = (size_t)sm_count() * 64;
+    if (blocks > cap) blocks = cap;
+    weights_generic_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(ref, w_out, dm);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "weights launch");
+}
+
+int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out,
+                                  int32_t z_begin, int32_t z_end, void *ws, size_t ws_bytes, void *cuda_stream,
+                                  int variant)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!f || !g || !f_out) return TNLM_ERR_NULL_POINTER;
+    if (z_begin < 0 || z_end > p->nz || z_begin > z_end) return TNLM_ERR_BAD_DIMS;
+    const int v = pick_variant(p, variant);
+    if (v < 0) return TNLM_ERR_UNSUPPORTED;
+    if (!ref) ref = f;
+    const size_t sb = stack_bytes(p);
+    if (misaligned(f) || misaligned(g) || misaligned(ref) || misaligned(f_out)) return TNLM_ERR_WORKSPACE;
+    if (overlaps(f_out, sb, f, sb) || overlaps(f_out, sb, g, sb) || overlaps(f_out, sb, ref, sb)) return TNLM_ERR_ALIAS;
+    rc = check_ws(p, ws, ws_bytes);
+    if (rc) return rc;
+    if (overlaps(ws, ws_bytes, f_out, sb) || overlaps(ws, ws_bytes, f, sb) || overlaps(ws, ws_bytes, g, sb) ||
+        overlaps(ws, ws_bytes, ref, sb))
+        return TNLM_ERR_ALIAS;
+    char *kws = (char *)ws + align_up(sb, 256);
+    return launch_sweep(p, f, g, ref, f_out, z_begin, z_end, kws, ws_bytes - align_up(sb, 256),
+                        (cudaStream_t)cuda_stream, v);
+}
+
+int tnlm_jacobi_step_slab(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out,
+                          int32_t z_begin, int32_t z_end, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    return tnlm_jacobi_step_slab_variant(p, f, g, ref, f_out, z_begin, z_end, ws, ws_bytes, cuda_stream,
+                                         TNLM_VARIANT_AUTO);
+}
+
+int tnlm_jacobi_step_variant(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out,
+                             void *ws, size_t ws_bytes, void *cuda_stream, int variant)
+{
+    if (!p) return TNLM_ERR_NULL_POINTER;
+    return tnlm_jacobi_step_slab_variant(p, f, g, ref, f_out, 0, p->nz, ws, ws_bytes, cuda_stream, variant);
+}
+
+int tnlm_jacobi_step(const tnlm_params *p, const float *f, const float *g, const float *ref, float *f_out, void *ws,
+                     size_t ws_bytes, void *cuda_stream)
+{
+    return tnlm_jacobi_step_variant(p, f, g, ref, f_out, ws, ws_bytes, cuda_stream, TNLM_VARIANT_AUTO);
+}
+
+int tnlm_enhance_variant(const tnlm_params *p, const float *g, const float *f_init, float *f_out, int32_t n_iter,
+                         void *ws, size_t ws_bytes, void *cuda_stream, int variant)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!g || !f_out) return TNLM_ERR_NULL_POINTER;
+    if (n_iter < 0) return TNLM_ERR_BAD_PARAM;
+    const int v = pick_variant(p, variant);
+    if (v < 0) return TNLM_ERR_UNSUPPORTED;
+    const size_t sb = stack_bytes(p);
+    if (misaligned(g) || misaligned(f_init) || misaligned(f_out)) return TNLM_ERR_WORKSPACE;
+    if (overlaps(f_out, sb, g, sb) || overlaps(f_out, sb, f_init, sb)) return TNLM_ERR_ALIAS;
+    rc = check_ws(p, ws, ws_bytes);
+    if (rc) return rc;
+    if (overlaps(ws, ws_bytes, f_out, sb) || overlaps(ws, ws_bytes, g, sb) || overlaps(ws, ws_bytes, f_init, sb))
+        return TNLM_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const float *cur = f_init ? f_init : g;   // f^0
+    if (n_iter == 0) {
+        cudaError_t e = cudaMemcpyAsync(f_out, cur, sb, cudaMemcpyDeviceToDevice, st);
+        return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "enhance copy");
+    }
+    float *buf_ws = (float *)ws;
+    char *kws = (char *)ws + align_up(sb, 256);
+    const size_t kws_bytes = ws_bytes - align_up(sb, 256);
+    // ping-pong between f_out and the workspace buffer so that the last sweep lands in f_out
+    float *dst = (n_iter % 2 == 1) ? f_out : buf_ws;
+    for (int k = 0; k < n_iter; ++k) {
+        // weights from the latest iterate f^k (ref = f^k), one sweep of Eq. 8
+        rc = launch_sweep(p, cur, g, cur, dst, 0, p->nz, kws, kws_bytes, st, v);
+        if (rc) return rc;
+        cur = dst;
+        dst = (dst == f_out) ? buf_ws : f_out;
+    }
+    return TNLM_OK;
+}
+
+int tnlm_enhance(const tnlm_params *p, const float *g, const float *f_init, float *f_out, int32_t n_iter, void *ws,
+                 size_t ws_bytes, void *cuda_stream)
+{
+    return tnlm_enhance_variant(p, g, f_init, f_out, n_iter, ws, ws_bytes, cuda_stream, TNLM_VARIANT_AUTO);
+}
+
+int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
+                      int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!g_host || !f_out_host) return TNLM_ERR_NULL_POINTER;
+    if (n_iter < 0) return TNLM_ERR_BAD_PARAM;
+    if (!dev_ws || misaligned(dev_ws) || dev_ws_bytes < tnlm_host_workspace_bytes(p)) return TNLM_ERR_WORKSPACE;
+    const size_t sb = stack_bytes(p), sba = align_up(sb, 256);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float *g_dev = (float *)dev_ws;
+    float *fi_dev = (float *)((char *)dev_ws + sba);
+    float *fo_dev = (float *)((char *)dev_ws + 2 * sba);
+    void *ws = (char *)dev_ws + 3 * sba;
+    cudaError_t e = cudaMemcpyAsync(g_dev, g_host, sb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "H2D g");
+    if (f_init_host) {
+        e = cudaMemcpyAsync(fi_dev, f_init_host, sb, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(e, "H2D f_init");
+    }
+    rc = tnlm_enhance(p, g_dev, f_init_host ? fi_dev : nullptr, fo_dev, n_iter, ws, dev_ws_bytes - 3 * sba, st);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(f_out_host, fo_dev, sb, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(e, "D2H f_out");
+    e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "enhance_host sync");
+}
+
+const char *tnlm_strerror(int code)
+{
+    switch (code) {
+        case TNLM_OK: return "ok";
+        case TNLM_ERR_NULL_POINTER: return "a required pointer is NULL";
+        case TNLM_ERR_BAD_DIMS: return "bad dimensions (extent < 1, n_phase < 2, slab out of range or stack too large)";
+        case TNLM_ERR_BAD_PARAM: return "bad parameter (h, mu not finite or <= 0; negative radius; n_iter < 0)";
+        case TNLM_ERR_UNSUPPORTED: return "radius or kernel variant not compiled in";
+        case TNLM_ERR_ALIAS: return "output overlaps an input or the workspace";
+        case TNLM_ERR_WORKSPACE: return "workspace or stack pointer NULL, too small or not 16-byte aligned";
+        case TNLM_ERR_CUDA: return g_cuda_err;
+        default: return "unknown tnlm status";
+    }
+}
+
+const char *tnlm_kernel_name(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return "invalid";
+    return tiled_supported(*p) ? tiled_name(*p) : "jacobi_generic_kernel";
+}
+
+int32_t tnlm_launches_per_sweep(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return 0;
+    return tiled_supported(*p) ? tiled_launches_per_sweep(*p) : 1;
+}
+
+int tnlm_probe_fp32(int32_t n_iter, float *sink, void *cuda_stream)
+{
+    if (!sink) return TNLM_ERR_NULL_POINTER;
+    if (n_iter < 0) return TNLM_ERR_BAD_PARAM;
+    fp32_probe_kernel<<<sm_count() * kProbeBlocksPerSM, kProbeThreads, 0, (cudaStream_t)cuda_stream>>>(
+        n_iter, sink, 0.999f, 0.001f);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "fp32 probe launch");
+}
+
+double tnlm_probe_fp32_ffma_count(int32_t n_iter)
+{
+    return (double)sm_count() * kProbeBlocksPerSM * kProbeThreads * (double)kProbeChains * (double)n_iter;
+}
+
+}  // extern "C"

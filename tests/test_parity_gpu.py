@@ -1,0 +1,234 @@
+"""Parity of the CUDA path (through the C ABI of libtnlm.so) with the CPU oracle, element by
+element on the same seeded inputs.  Bar (BASELINE.json north_star):
+    max |delta| <= 1e-4 * (max g - min g)    and    ||delta||_2 / ||f_oracle||_2 <= 1e-5   in fp32.
+"""
+import numpy as np
+import pytest
+
+from tnlm_inputs import CONFIGS, make_stack, dynamic_range, random_stack
+
+pytestmark = pytest.mark.gpu
+
+MAX_TOL = 1e-4     # x dynamic range of the input
+L2_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    import paper_1201_2450_b200 as T
+    T.lib()   # fails loudly if libtnlm.so is missing: there is no fallback
+    return T
+
+
+def variants(T, p):
+    out = [T.VARIANT_GENERIC]
+    if T.kernel_name(p) != "jacobi_generic_kernel":
+        out.append(T.VARIANT_TILED)
+    return out
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def assert_parity(got, want, rng_scale, what=""):
+    got = np.asarray(got, dtype=np.float64)
+    want = np.asarray(want, dtype=np.float64)
+    assert np.isfinite(got).all(), f"{what}: non-finite output"
+    max_err = np.abs(got - want).max()
+    l2 = np.linalg.norm(got - want) / max(np.linalg.norm(want), 1e-300)
+    assert max_err <= MAX_TOL * rng_scale, f"{what}: max|d|={max_err:.3e} > {MAX_TOL * rng_scale:.3e}"
+    assert l2 <= L2_TOL, f"{what}: rel L2={l2:.3e} > {L2_TOL}"
+    return max_err, l2
+
+
+def params_of(T, cfg, shape=None):
+    return T.TnlmParams.make(shape or cfg.shape, cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+
+
+# ------------------------------------------------------------------ config 1: full trajectory
+def test_config1_full_enhancement(T, oracle):
+    cfg = CONFIGS["config1"]
+    g = make_stack(cfg)
+    p = params_of(T, cfg)
+    want = oracle.enhance(g, cfg.patch_radius, cfg.search_radius, np.float32(cfg.h), np.float32(cfg.mu), cfg.n_iter)
+    for v in variants(T, p):
+        got = T.tnlm_enhance(p, dev(g), cfg.n_iter, variant=v).cpu().numpy()
+        assert_parity(got, want, dynamic_range(g), f"config1 variant {v}")
+
+
+# ------------------------------------------------------------------ config 2 recipe, reduced grid
+def test_config2_recipe_reduced_two_sweeps(T, oracle):
+    """Thorax recipe of config 2 (d=1, M=2, h=0.05, mu=0.5) on a grid the oracle finishes in
+    seconds; extents span several tiles and leave ragged tails in x, y and z."""
+    cfg = CONFIGS["config2"].scaled(nz=21, ny=45, nx=70, n_phase=4, tumour_radius=3, si_amplitude=3)
+    g = make_stack(cfg)
+    p = params_of(T, cfg)
+    want = oracle.enhance(g, 1, 2, np.float32(cfg.h), np.float32(cfg.mu), 2)
+    for v in variants(T, p):
+        got = T.tnlm_enhance(p, dev(g), 2, variant=v).cpu().numpy()
+        assert_parity(got, want, dynamic_range(g), f"config2-reduced variant {v}")
+
+
+# ------------------------------------------------------------------ edge cases
+EDGE = [
+    # shape,            d, M, h,     mu
+    ((2, 1, 1, 1),      1, 1, 0.1,   1.0),    # smallest legal stack, P=2 counts the neighbour twice
+    ((2, 3, 4, 5),      1, 2, 0.05,  0.5),    # window larger than the volume
+    ((3, 5, 7, 9),      0, 1, 0.1,   1.0),    # d=0: single-voxel patch
+    ((3, 5, 7, 9),      1, 0, 0.1,   1.0),    # M=0: closed form (mu g + f+ + f-)/(2+mu)
+    ((3, 6, 9, 33),     2, 1, 0.2,   0.3),    # 5^3 patch
+    ((3, 9, 11, 37),    1, 3, 0.06,  0.5),    # 7^3 window (config 4's)
+    ((3, 9, 10, 35),    2, 2, 0.1,   0.5),
+    ((2, 10, 12, 34),   1, 4, 0.1,   2.0),    # 9^3 window
+    ((5, 2, 31, 129),   1, 2, 0.05,  0.5),    # flat slab, ragged x
+    ((3, 17, 3, 4),     1, 1, 0.02,  0.5),    # tiny h: exponents in the thousands (reading P3)
+    ((3, 4, 5, 6),      3, 1, 0.5,   0.5),    # largest compiled patch radius
+]
+
+
+@pytest.mark.parametrize("shape,d,M,h,mu", EDGE)
+def test_edge_cases_one_sweep(T, oracle, shape, d, M, h, mu):
+    f = random_stack(shape, 7)
+    g = random_stack(shape, 8)
+    p = T.TnlmParams.make(shape, d, M, h, mu)
+    want = oracle.jacobi_step(f, g, d, M, np.float32(h), np.float32(mu))
+    for v in variants(T, p):
+        got = T.tnlm_jacobi_step(p, dev(f), dev(g), variant=v).cpu().numpy()
+        assert_parity(got, want, 1.0, f"edge {shape} d={d} M={M} variant {v}")
+
+
+def test_separate_ref_stack(T, oracle):
+    """TNLM-R usage: weights from ref = g^(k), averages of f."""
+    shape = (3, 9, 20, 41)
+    f, g, ref = random_stack(shape, 1), random_stack(shape, 2), random_stack(shape, 3)
+    p = T.TnlmParams.make(shape, 1, 2, 0.3, 0.5)
+    want = oracle.jacobi_step(f, g, 1, 2, np.float32(0.3), np.float32(0.5), ref=ref)
+    for v in variants(T, p):
+        got = T.tnlm_jacobi_step(p, dev(f), dev(g), ref=dev(ref), variant=v).cpu().numpy()
+        assert_parity(got, want, 1.0, f"separate ref variant {v}")
+
+
+def test_constant_stack_is_fixed_point_and_bounds(T):
+    import torch
+    shape = (4, 9, 33, 65)
+    p = T.TnlmParams.make(shape, 1, 2, 0.05, 0.5)
+    c = torch.full(shape, 0.3125, device="cuda")
+    g = dev(random_stack(shape, 11))
+    for v in variants(T, p):
+        out = T.tnlm_jacobi_step(p, c, c, variant=v)
+        assert (out - c).abs().max().item() <= 1e-6
+        f = T.tnlm_enhance(p, g, 3, variant=v)
+        assert f.min().item() >= g.min().item() - 1e-6 and f.max().item() <= g.max().item() + 1e-6
+
+
+def test_weights_match_oracle(T, oracle):
+    shape = (3, 4, 6, 10)
+    ref = random_stack(shape, 21)
+    p = T.TnlmParams.make(shape, 1, 1, 0.2, 1.0)
+    want = oracle.weights(ref, 1, 1, np.float32(0.2))
+    got = T.tnlm_weights(p, dev(ref)).cpu().numpy()
+    assert got.shape == want.shape and (got >= 0).all()
+    np.testing.assert_allclose(got.sum(axis=2), 1.0, atol=2e-6)
+    np.testing.assert_allclose(got, want, rtol=0, atol=2e-5)
+
+
+# ------------------------------------------------------------------ loop / ABI semantics on the device
+def test_enhance_equals_manual_steps_bitwise(T):
+    import torch
+    cfg = CONFIGS["config1"]
+    g = dev(make_stack(cfg))
+    p = params_of(T, cfg)
+    for v in variants(T, p):
+        f = g
+        for _ in range(3):
+            f = T.tnlm_jacobi_step(p, f, g, variant=v)
+        assert torch.equal(T.tnlm_enhance(p, g, 3, variant=v), f)
+        assert torch.equal(T.tnlm_enhance(p, g, 0, variant=v), g)
+        f1 = T.tnlm_enhance(p, g, 1, variant=v)
+        assert torch.equal(T.tnlm_enhance(p, g, 2, f_init=f1, variant=v), f)
+        assert torch.equal(T.tnlm_enhance(p, g, 4, variant=v), T.tnlm_jacobi_step(p, f, g, variant=v))
+
+
+def test_slabs_tile_the_sweep_bitwise(T):
+    import torch
+    shape = (3, 19, 30, 40)
+    f, g = dev(random_stack(shape, 31)), dev(random_stack(shape, 32))
+    p = T.TnlmParams.make(shape, 1, 2, 0.1, 0.5)
+    for v in variants(T, p):
+        full = T.tnlm_jacobi_step(p, f, g, variant=v)
+        out = torch.full_like(f, -7.0)
+        for (a, b) in [(0, 5), (5, 6), (6, 6), (6, 19)]:
+            T.tnlm_jacobi_step_slab(p, f, g, a, b, f_out=out, variant=v)
+        assert torch.equal(out, full)
+
+
+def test_enhance_host_matches_device_path(T):
+    import torch
+    cfg = CONFIGS["config1"]
+    g = make_stack(cfg)
+    p = params_of(T, cfg)
+    gh = torch.from_numpy(g).pin_memory()
+    out_h = T.tnlm_enhance_host(p, gh, cfg.n_iter)
+    out_d = T.tnlm_enhance(p, dev(g), cfg.n_iter)
+    assert torch.equal(out_h, out_d.cpu())
+
+
+def test_device_error_codes(T):
+    import torch
+    shape = (3, 4, 8, 8)
+    p = T.TnlmParams.make(shape, 1, 1, 0.1, 1.0)
+    f = torch.rand(shape, device="cuda")
+    with pytest.raises(T.TnlmError) as e:
+        T.tnlm_jacobi_step(p, f, f, f_out=f)
+    assert e.value.code == -5
+    with pytest.raises(T.TnlmError) as e:
+        T.tnlm_jacobi_step(p, f, f, ws=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -6
+    bad = T.TnlmParams.make(shape, 1, 1, 0.0, 1.0)
+    with pytest.raises(T.TnlmError) as e:
+        T.tnlm_jacobi_step(bad, f, f)
+    assert e.value.code == -3
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration
+def _sampled_step_parity(T, oracle, cfg, n_samples, what):
+    import torch
+    g = make_stack(cfg)
+    p = params_of(T, cfg)
+    gd = dev(g)
+    ws = torch.empty(T.workspace_bytes(p), dtype=torch.uint8, device="cuda")
+    f1 = T.tnlm_jacobi_step(p, gd, gd, ws=ws)                 # first sweep: f^0 = g
+    f2 = T.tnlm_jacobi_step(p, f1, gd, ws=ws)                 # second sweep from the GPU's own f^1
+    rng = np.random.default_rng(5)
+    P, Z, Y, X = cfg.shape
+    idx = rng.integers(0, g.size, n_samples)
+    # add corners, faces and the last voxel: where clamping and ragged tiles live
+    extra = [0, g.size - 1, X - 1, (Y - 1) * X, (Z - 1) * Y * X, Y * X * Z - 1, Y * X * Z, 2 * Y * X * Z - 1]
+    idx = np.unique(np.concatenate([idx, np.array(extra, dtype=np.int64)]))
+    h, mu = np.float32(cfg.h), np.float32(cfg.mu)
+    f1h = f1.cpu().numpy()
+    want1 = oracle.jacobi_step_at(g, g, cfg.patch_radius, cfg.search_radius, h, mu, idx)
+    want2 = oracle.jacobi_step_at(f1h, g, cfg.patch_radius, cfg.search_radius, h, mu, idx)
+    rs = dynamic_range(g)
+    assert_parity(f1h.reshape(-1)[idx], want1, rs, what + " sweep 1")
+    assert_parity(f2.cpu().numpy().reshape(-1)[idx], want2, rs, what + " sweep 2 (step-wise)")
+    assert f2.min().item() >= g.min() - 1e-6 and f2.max().item() <= g.max() + 1e-6
+
+
+def test_config3_full_size_sampled(T, oracle):
+    """10 x 128 x 256 x 256, the configuration bench.py times: oracle at sampled output voxels."""
+    _sampled_step_parity(T, oracle, CONFIGS["config3"], 6000, "config3")
+
+
+def test_config2_full_size_sampled(T, oracle):
+    _sampled_step_parity(T, oracle, CONFIGS["config2"], 6000, "config2")
+
+
+def test_config4_shape_sampled(T, oracle):
+    """Clinical-scale recipe (7^3 window, Z = 100 not a power of two) on a quarter in-plane grid."""
+    cfg = CONFIGS["config4"].scaled(ny=256, nx=256, tumour_radius=8, si_amplitude=6)
+    _sampled_step_parity(T, oracle, cfg, 3000, "config4 (256x256x100)")
