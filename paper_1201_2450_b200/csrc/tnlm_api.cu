@@ -145,9 +145,13 @@ int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const fl
     if (rc) return rc;
     if (!f || !g || !f_out) return TNLM_ERR_NULL_POINTER;
     if (z_begin < 0 || z_end > p->nz || z_begin > z_end) return TNLM_ERR_BAD_DIMS;
-    const int v = pick_variant(p, variant);
+    int v = pick_variant(p, variant);
     if (v < 0) return TNLM_ERR_UNSUPPORTED;
     if (!ref) ref = f;
+    if (v == TNLM_VARIANT_TILED && ref != f) {   // the tiled kernel covers TNLM-E (ref = f) only
+        if (variant == TNLM_VARIANT_TILED) return TNLM_ERR_UNSUPPORTED;
+        v = TNLM_VARIANT_GENERIC;
+    }
     const size_t sb = stack_bytes(p);
     if (misaligned(f) || misaligned(g) || misaligned(ref) || misaligned(f_out)) return TNLM_ERR_WORKSPACE;
     if (overlaps(f_out, sb, f, sb) || overlaps(f_out, sb, g, sb) || overlaps(f_out, sb, ref, sb)) return TNLM_ERR_ALIAS;

@@ -107,9 +107,14 @@ def test_separate_ref_stack(T, oracle):
     f, g, ref = random_stack(shape, 1), random_stack(shape, 2), random_stack(shape, 3)
     p = T.TnlmParams.make(shape, 1, 2, 0.3, 0.5)
     want = oracle.jacobi_step(f, g, 1, 2, np.float32(0.3), np.float32(0.5), ref=ref)
-    for v in variants(T, p):
+    # the tiled kernel covers ref = f only: AUTO falls back to the generic kernel, an explicit request is refused
+    for v in (T.VARIANT_GENERIC, T.VARIANT_AUTO):
         got = T.tnlm_jacobi_step(p, dev(f), dev(g), ref=dev(ref), variant=v).cpu().numpy()
         assert_parity(got, want, 1.0, f"separate ref variant {v}")
+    if T.VARIANT_TILED in variants(T, p):
+        with pytest.raises(T.TnlmError) as e:
+            T.tnlm_jacobi_step(p, dev(f), dev(g), ref=dev(ref), variant=T.VARIANT_TILED)
+        assert e.value.code == -4
 
 
 def test_constant_stack_is_fixed_point_and_bounds(T):
