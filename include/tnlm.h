@@ -54,7 +54,7 @@ typedef enum {
 } tnlm_status;
 
 /* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M). */
-enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2 };
+enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2, TNLM_VARIANT_PAIRED = 3 };
 
 /*
  * Bytes of caller-owned device workspace that tnlm_jacobi_step / tnlm_enhance / tnlm_weights need

@@ -7,6 +7,7 @@
 #include "tnlm_common.cuh"
 #include "tnlm_generic.cuh"
 #include "tnlm_tiled.cuh"
+#include "tnlm_pair.cuh"
 
 namespace {
 
@@ -60,7 +61,8 @@ int pick_variant(const tnlm_params *p, int variant)
 {
     if (variant == TNLM_VARIANT_GENERIC) return TNLM_VARIANT_GENERIC;
     if (variant == TNLM_VARIANT_TILED) return tiled_supported(*p) ? TNLM_VARIANT_TILED : -1;
-    if (variant == TNLM_VARIANT_AUTO) return tiled_supported(*p) ? TNLM_VARIANT_TILED : TNLM_VARIANT_GENERIC;
+    if (variant == TNLM_VARIANT_PAIRED) return pair_supported(*p) ? TNLM_VARIANT_PAIRED : -1;
+    if (variant == TNLM_VARIANT_AUTO) return pair_supported(*p) ? TNLM_VARIANT_PAIRED : TNLM_VARIANT_GENERIC;
     return -1;
 }
 
@@ -70,6 +72,10 @@ int launch_sweep(const tnlm_params *p, const float *f, const float *g, const flo
 {
     if (z1 <= z0) return TNLM_OK;
     const Dims dm = make_dims(*p, z0, z1);
+    if (variant == TNLM_VARIANT_PAIRED) {
+        cudaError_t e = launch_pair(*p, dm, f, g, ref, f_out, st);
+        return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "paired sweep launch");
+    }
     if (variant == TNLM_VARIANT_TILED) {
         cudaError_t e = launch_tiled(*p, dm, f, g, ref, f_out, kernel_ws, kernel_ws_bytes, st);
         return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "tiled sweep launch");
@@ -148,8 +154,8 @@ int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const fl
     int v = pick_variant(p, variant);
     if (v < 0) return TNLM_ERR_UNSUPPORTED;
     if (!ref) ref = f;
-    if (v == TNLM_VARIANT_TILED && ref != f) {   // the tiled kernel covers TNLM-E (ref = f) only
-        if (variant == TNLM_VARIANT_TILED) return TNLM_ERR_UNSUPPORTED;
+    if ((v == TNLM_VARIANT_TILED || v == TNLM_VARIANT_PAIRED) && ref != f) {   // these cover TNLM-E (ref = f) only
+        if (variant != TNLM_VARIANT_AUTO) return TNLM_ERR_UNSUPPORTED;
         v = TNLM_VARIANT_GENERIC;
     }
     const size_t sb = stack_bytes(p);
@@ -274,13 +280,13 @@ const char *tnlm_strerror(int code)
 const char *tnlm_kernel_name(const tnlm_params *p)
 {
     if (check_params(p) != TNLM_OK) return "invalid";
-    return tiled_supported(*p) ? tiled_name(*p) : "jacobi_generic_kernel";
+    return pair_supported(*p) ? pair_name(*p) : "jacobi_generic_kernel";
 }
 
 int32_t tnlm_launches_per_sweep(const tnlm_params *p)
 {
     if (check_params(p) != TNLM_OK) return 0;
-    return tiled_supported(*p) ? tiled_launches_per_sweep(*p) : 1;
+    return 1;
 }
 
 int tnlm_probe_fp32(int32_t n_iter, float *sink, void *cuda_stream)

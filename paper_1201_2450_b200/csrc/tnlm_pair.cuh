@@ -1,0 +1,469 @@
+// Row-pair packed sm_100a TNLM sweep kernel for 3^3 patches (d = 1), search radius M in {1,2,3,4}.
+//
+// Blackwell's FP32 pipe executes FADD2 / FMUL2 / FFMA2 (two fp32 lanes of a 64-bit register pair per
+// thread) at the same lane rate as the scalar forms but for half the issue slots; the scalar tiled
+// kernel (tnlm_tiled.cuh) is issue bound.  Here every value of the distance pipeline is a float2 that
+// holds the SAME quantity for two vertically adjacent voxels (rows 2l and 2l+1 of the tile), so a1-a4
+// all run packed, and each thread needs one shuffle per output for the y-sum instead of two.
+//
+// One CTA = one (phase i, TX-wide x-tile, 30-row y-group, RZ-plane z-slab), both neighbour phases in turn
+// (Eq. 8).  Shared memory holds float2 row-pair tiles:
+//   A2 [RZ+2   ][16  ][PA2]   -ref_i, pair k = tile rows (2k, 2k+1), halo d = 1 (stored negated: a1 is an add)
+//   BE [RZ+2+2M][16+M][PB2]    ref_j, pair k = tile rows (2k,   2k+1)   used when the y-offset is even
+//   BO [RZ+2+2M][16+M][PB2]    ref_j, pair k = tile rows (2k+1, 2k+2)   used when the y-offset is odd
+// (clamp-to-edge applied while staging: reading P4).  The second copy of B keeps the operand of every
+// packed op an aligned register pair for any y-offset.
+//
+//   half-warp   = 16 lanes = 16 row pairs = 32 tile rows (rows 0 and 31 are the d-halo: 30 output rows)
+//   thread      = 2 rows x an x-run of 2 voxels x a column of RZ output planes = 4*RZ outputs
+//   registers   = (Z, N, reference exponent) of its outputs for the whole search window
+//   per (ty,tz) = a "pass": march the RZ+2 planes; per plane, for W consecutive tx at once
+//       a1  d = b + (-a)                                      FADD2, operands straight from LDS.128 windows
+//       a2x 3-tap x-sum of squares; the two outputs share the middle pair    FMUL2 + 3 FFMA2 per 2 outputs
+//       a2z 3-tap z-sum from a two-plane register ring                       2 FADD2
+//       a2y S.lo + S.hi (own two rows) + one row from the lane above / below  1 FADD + 2 SHFL + 1 FADD2
+//       a3  u = ex2(bias - c2*D)                                              FFMA2 + 2 MUFU.EX2
+//       a4  Z += u, N += u * f_j(x+t)                                         FADD2 + FFMA2
+//   epilogue    = NLM of the first direction is parked in f_out (same thread reads it back), then
+//                 a5: f_out = mu/(2+mu) g + (NLM- + NLM+)/(2+mu)
+// Reference exponent (reading P3: weights relative to the best candidate).  The first pass (zero y/z
+// offset) sets the reference exponent of every output from its best candidate; later passes add their
+// terms optimistically and check the partial normaliser against a 2^100 guard band.  Row pairs whose
+// terms left the band (a candidate > 2^100 times better than the reference: moving high-contrast edges)
+// are not added; the thread re-does them in pair_cold (direct 27-tap distances, re-base, add).  The
+// result equals the shifted softmax up to rounding.
+#pragma once
+#include <cstdlib>
+
+#include "tnlm_common.cuh"
+#include "tnlm_tiled.cuh"
+
+namespace tnlm {
+
+constexpr int kPairRowsOut = 30;
+
+__host__ __device__ constexpr int pitch2(int n)   // smallest p >= n with p = 2 (mod 4): conflict-free LDS.128
+{
+    int p = n;
+    while (p % 4 != 2) ++p;
+    return p;
+}
+
+__device__ __forceinline__ float2 add2(const float2 a, const float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 mul2(const float2 a, const float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(const float2 a, const float2 b, const float2 c) { return __ffma2_rn(a, b, c); }
+
+template <int M, int RZ, int TX> struct PairGeom {
+    using C = Chunks<M>;
+    static constexpr int E = 2 * M + 1;
+    static constexpr int NRUN = TX / 2;             // x-runs of 2 voxels
+    static constexpr int NT = NRUN * 16;            // 16 row-pair lanes per run
+    static constexpr int NVB0 = (C::W0 + 4) / 2;    // LDS.128 per B row window (2 + W + 1 positions)
+    static constexpr int NVB1 = C::W1 ? (C::W1 + 4) / 2 : 0;
+    static constexpr int ACOLS = TX + 2, BCOLS = TX + 2 * M + 2;   // staged columns
+    static constexpr int BREAD = cmax(TX - 2 + 2 * NVB0, C::W1 ? TX - 2 + 4 + 2 * NVB1 : 0);   // columns a window may touch
+    static constexpr int PA2 = pitch2(ACOLS);
+    static constexpr int PB2 = pitch2(cmax(BCOLS, BREAD));
+    static constexpr int NPA = 16, NPE = 16 + M, NPO = 16 + M;     // row pairs per plane (BO padded: same plane stride as BE)
+    static constexpr int NAP = RZ + 2, NBP = RZ + 2 + 2 * M;       // planes
+    static constexpr int A_F2 = NAP * NPA * PA2, BE_F2 = NBP * NPE * PB2, BO_F2 = NBP * NPO * PB2;
+    static constexpr size_t BYTES = (size_t)(A_F2 + BE_F2 + BO_F2) * sizeof(float2);
+};
+
+struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
+
+constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100: Z stays below 2^107 (safe for __fdividef)
+
+template <int NV>
+__device__ __forceinline__ void load_pairs(const float2 *__restrict__ p, float2 (&dst)[2 * NV])
+{
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const float4 t = *reinterpret_cast<const float4 *>(p + 2 * v);
+        dst[2 * v] = make_float2(t.x, t.y);
+        dst[2 * v + 1] = make_float2(t.z, t.w);
+    }
+}
+
+// One pass: W consecutive x-offsets at fixed (ty, tz), marching the RZ+2 planes.
+//   aRow: &A2[plane 0][pair l][x0]                 element k <-> x = X0 + x0 - 1 + k   (negated values)
+//   bRow: &B?[plane tz][pair l + ty/2][x0 + q0]    element k + q pairs with a[k] for the q-th offset of the chunk
+// FIRST: the accumulators are empty; the reference exponent of every output is set from the best
+//        candidate of this pass (exact, no guard needed).
+// else : optimistic add; returns a bit mask (bit 2*o + i) of the row pairs whose terms left the guard
+//        band and were NOT added (the caller sends those through pair_cold).
+template <int RZ, int W, bool FIRST, int A_PLANE, int B_PLANE>
+__device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
+                                              const float c2, AccPair (&acc)[RZ])
+{
+    constexpr int NVB = (W + 4) / 2;
+    const float2 nc2 = make_float2(-c2, -c2);
+    float2 ring0[W][2], ring1[W][2];
+    float2 bprev[2 * NVB];
+    unsigned fail = 0u;
+#pragma unroll
+    for (int p = 0; p < RZ + 2; ++p) {
+        float2 a[4], b[2 * NVB];
+        load_pairs<2>(aRow + p * A_PLANE, a);
+        load_pairs<NVB>(bRow + p * B_PLANE, b);
+        float2 X[W][2];
+#pragma unroll
+        for (int q = 0; q < W; ++q) {
+            float2 d[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) d[k] = add2(b[k + q], a[k]);                      // a1 (a is -ref_i)
+            const float2 mid = fma2(d[2], d[2], mul2(d[1], d[1]));                        // a2x
+            X[q][0] = fma2(d[0], d[0], mid);
+            X[q][1] = fma2(d[3], d[3], mid);
+        }
+        if (p >= 2) {
+            AccPair &ac = acc[p - 2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                float2 D[W];
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    const float2 S = add2(add2(ring0[q][i], ring1[q][i]), X[q][i]);       // a2z
+                    const float own = S.x + S.y;                                          // a2y
+                    const float up = __shfl_up_sync(0xffffffffu, S.y, 1);                 // row 2l-1
+                    const float dn = __shfl_down_sync(0xffffffffu, S.x, 1);               // row 2l+2
+                    D[q] = add2(make_float2(up, dn), make_float2(own, own));
+                }
+                if (FIRST) {
+                    float2 dmin = D[0];
+#pragma unroll
+                    for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
+                    ac.b[i] = make_float2(c2 * dmin.x, c2 * dmin.y);
+                }
+                float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int q = 0; q < W; ++q) {
+                    const float2 arg = fma2(D[q], nc2, ac.b[i]);                          // a3
+                    const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
+                    zp = add2(zp, u);                                                     // a4
+                    np = fma2(u, bprev[i + 1 + q], np);
+                }
+                if (FIRST) {
+                    ac.z[i] = zp;
+                    ac.n[i] = np;
+                } else if (fmaxf(zp.x, zp.y) <= kPairGuard) {
+                    ac.z[i] = add2(ac.z[i], zp);
+                    ac.n[i] = add2(ac.n[i], np);
+                } else {
+                    fail |= 1u << (2 * (p - 2) + i);
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < W; ++q)
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                ring0[q][i] = ring1[q][i];
+                ring1[q][i] = X[q][i];
+            }
+#pragma unroll
+        for (int k = 0; k < 2 * NVB; ++k) bprev[k] = b[k];
+    }
+    return fail;
+}
+
+// Cold path: re-do the W terms of the flagged row pairs (bit 2*o + i of `fail`) with distances taken
+// directly from the tiles, re-basing an output on its best candidate when that beats its reference.
+//   accl: the thread's accumulators, [(2*o + i)*6 + {z.x, z.y, n.x, n.y, b.x, b.y}]
+template <int M, int RZ, int TX>
+__device__ __noinline__ void pair_cold(float *accl, unsigned fail, const float *__restrict__ sA,
+                                       const float *__restrict__ sBE, const int l, const int x0, const int q0,
+                                       const int W, const int ty, const int tz, const float c2)
+{
+    using G = PairGeom<M, RZ, TX>;
+    while (fail) {
+        const int bit = __ffs(fail) - 1;
+        fail &= fail - 1;
+        const int o = bit >> 1, i = bit & 1;
+        float *ac = accl + bit * 6;
+#pragma unroll 1
+        for (int e = 0; e < 2; ++e) {
+            const int r = 2 * l + e;
+            float D[5], v[5];
+            float Dmin = INFINITY;
+#pragma unroll 1
+            for (int q = 0; q < W; ++q) {
+                float acc = 0.f;
+                for (int dz = -1; dz <= 1; ++dz)
+                    for (int dy = -1; dy <= 1; ++dy) {
+                        const int ra = min(max(r + dy, 0), 31), rb = min(max(r + ty + dy, 0), 31 + 2 * M);
+                        const float *pa = sA + (((o + 1 + dz) * G::NPA + (ra >> 1)) * G::PA2 + x0 + i + 1) * 2 + (ra & 1);
+                        const float *pb = sBE + (((o + 1 + tz + dz) * G::NPE + (rb >> 1)) * G::PB2 + x0 + i + 1 + q0 + q) * 2 + (rb & 1);
+                        for (int dx = -1; dx <= 1; ++dx) {
+                            const float d = pa[2 * dx] + pb[2 * dx];   // sA holds -ref_i
+                            acc = fmaf(d, d, acc);
+                        }
+                    }
+                const int rb = r + ty;
+                v[q] = sBE[(((o + 1 + tz) * G::NPE + (rb >> 1)) * G::PB2 + x0 + i + 1 + q0 + q) * 2 + (rb & 1)];
+                D[q] = acc;
+                Dmin = fminf(Dmin, acc);
+            }
+            float Z = ac[e], N = ac[2 + e], bias = ac[4 + e];
+            const float nb = c2 * Dmin;
+            if (nb < bias) {   // a better candidate than the reference: re-base
+                const float sc = ex2(nb - bias);
+                Z *= sc;
+                N *= sc;
+                bias = nb;
+            }
+#pragma unroll 1
+            for (int q = 0; q < W; ++q) {
+                const float u = ex2(fmaf(-c2, D[q], bias));
+                Z += u;
+                N = fmaf(u, v[q], N);
+            }
+            ac[e] = Z; ac[2 + e] = N; ac[4 + e] = bias;
+        }
+    }
+}
+
+// Stage a clamped halo tile into row-pair layout(s):
+//   tile element (pz, r, c) <- sign * src(clamp(zo+pz), clamp(yo+r), clamp(xo+c))
+//   dstE pair r/2 (half r&1); dstO (optional) pair (r-1)/2 (half (r-1)&1) for r >= 1
+// The (r, c) of a thread's k-th element is the same in every plane, so its global offset inside a
+// plane and its shared-memory offsets are tabulated once; the plane loop is then LDG + STS only,
+// two planes (2K loads) in flight per thread.
+template <int PITCH2, int ROWS, int COLS, int PLANES, int NP, bool ODD, bool NEGATE, int NT>
+__device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__restrict__ dstO,
+                                            const float *__restrict__ src, const int zo, const int yo, const int xo,
+                                            const Dims &dm, const int tid)
+{
+    constexpr int K = (ROWS * COLS + NT - 1) / NT;
+    constexpr int PLANE_F = NP * PITCH2 * 2;   // floats per shared-memory plane
+    int goff[K], eoff[K], ooff[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const int idx = tid + k * NT;
+        const int r = idx / COLS, c = idx - r * COLS;
+        const bool ok = idx < ROWS * COLS;
+        goff[k] = clampi(yo + r, dm.Y) * dm.X + clampi(xo + c, dm.X);
+        eoff[k] = ok ? (((r >> 1) * PITCH2 + c) * 2 + (r & 1)) : -1;
+        const int ro = r - 1;
+        ooff[k] = (ok && ro >= 0 && (ro >> 1) < NP) ? (((ro >> 1) * PITCH2 + c) * 2 + (ro & 1)) : -1;
+        if (!ok) goff[k] = 0;
+    }
+    const size_t plane = (size_t)dm.Y * dm.X;
+#pragma unroll 1
+    for (int pz = 0; pz < PLANES; pz += 2) {
+        float v[2][K];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const float *sp = src + (size_t)clampi(zo + min(pz + h, PLANES - 1), dm.Z) * plane;
+#pragma unroll
+            for (int k = 0; k < K; ++k) v[h][k] = __ldg(sp + goff[k]);
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (pz + h < PLANES) {
+                float *dE = dstE + (pz + h) * PLANE_F;
+                float *dO = dstO + (pz + h) * PLANE_F;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    const float val = NEGATE ? -v[h][k] : v[h][k];
+                    if (eoff[k] >= 0) dE[eoff[k]] = val;
+                    if (ODD && ooff[k] >= 0) dO[ooff[k]] = val;
+                }
+            }
+        }
+    }
+}
+
+template <int M, int RZ, int TX>
+__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, (PairGeom<M, RZ, TX>::NT <= 128) ? 2 : 1)
+tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float *f_out, const Dims dm,
+                 const int tiles_x, const int tiles_y, const int tiles_z)
+{
+    using G = PairGeom<M, RZ, TX>;
+    using C = Chunks<M>;
+    constexpr int AP = G::NPA * G::PA2, BP = G::NPE * G::PB2;   // plane strides (float2)
+    extern __shared__ __align__(16) float smem[];
+    float2 *sA = reinterpret_cast<float2 *>(smem);
+    float2 *sBE = sA + G::A_F2;
+    float2 *sBO = sBE + G::BE_F2;
+
+    int t = blockIdx.x;
+    const int bx = t % tiles_x; t /= tiles_x;
+    const int by = t % tiles_y; t /= tiles_y;
+    const int bz = t % tiles_z; t /= tiles_z;
+    const int ph = t;
+    const int X0 = bx * TX, Y0 = by * kPairRowsOut, Z0 = dm.z_begin + bz * RZ;
+    const size_t V = (size_t)dm.Z * dm.Y * dm.X;
+    const int tid = threadIdx.x;
+    const int l = tid & 15;            // row pair: tile rows 2l, 2l+1
+    const int x0 = 2 * (tid >> 4);     // first x of the run, tile relative
+
+    // -ref_i tile (halo 1): rows <-> y = Y0-1+r, cols <-> x = X0-1+c, planes <-> z = Z0-1+pz
+    stage_pairs<G::PA2, 32, G::ACOLS, G::NAP, G::NPA, false, true, G::NT>(
+        reinterpret_cast<float *>(sA), nullptr, f + (size_t)ph * V, Z0 - 1, Y0 - 1, X0 - 1, dm, tid);
+
+    const size_t zstride = (size_t)dm.Y * dm.X;
+    const bool vec_ok = (dm.X % 2) == 0;
+    const bool col_ok = X0 + x0 < dm.X;
+
+#pragma unroll 1
+    for (int s = 0; s < 2; ++s) {
+        const int j = (ph + (s ? 1 : dm.P - 1)) % dm.P;
+        __syncthreads();   // everyone is done with the previous B tiles
+        // f_j tiles (halo 1+M): rows <-> y = Y0-1-M+r, cols <-> x = X0-1-M+c, planes <-> z = Z0-1-M+pz
+        stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NBP, G::NPE, true, false, G::NT>(
+            reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), f + (size_t)j * V, Z0 - 1 - M, Y0 - 1 - M,
+            X0 - 1 - M, dm, tid);
+        __syncthreads();
+
+        AccPair acc[RZ];   // fully written by the first pass
+        const float2 *aRow = sA + l * G::PA2 + x0;
+        static_assert(G::NPE == G::NPO, "BE and BO share one plane stride");
+
+        // the thread's accumulators take a round trip through local memory around the (rare) cold path
+        auto run_cold = [&](unsigned fail, int q0, int W, int ty, int tz) {
+            float accl[RZ * 12];
+#pragma unroll
+            for (int o = 0; o < RZ; ++o)
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    float *a6 = accl + (2 * o + i) * 6;
+                    a6[0] = acc[o].z[i].x; a6[1] = acc[o].z[i].y;
+                    a6[2] = acc[o].n[i].x; a6[3] = acc[o].n[i].y;
+                    a6[4] = acc[o].b[i].x; a6[5] = acc[o].b[i].y;
+                }
+            pair_cold<M, RZ, TX>(accl, fail, reinterpret_cast<const float *>(sA), reinterpret_cast<const float *>(sBE), l,
+                                 x0, q0, W, ty, tz, dm.c2);
+#pragma unroll
+            for (int o = 0; o < RZ; ++o)
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const float *a6 = accl + (2 * o + i) * 6;
+                    acc[o].z[i] = make_float2(a6[0], a6[1]);
+                    acc[o].n[i] = make_float2(a6[2], a6[3]);
+                    acc[o].b[i] = make_float2(a6[4], a6[5]);
+                }
+        };
+
+        // first pass: (ty, tz) = zero offset; its first chunk sets every output's reference exponent
+        // (the zero offset is usually the best match, so the cold path stays cold)
+        {
+            const float2 *bRow = ((M & 1) ? sBO : sBE) + (M * G::NPE + l + (M >> 1)) * G::PB2 + x0;
+            pair_pass<RZ, C::W0, true, AP, BP>(aRow, bRow, dm.c2, acc);
+            if constexpr (C::W1 > 0) {
+                const unsigned fail = pair_pass<RZ, C::W1, false, AP, BP>(aRow, bRow + 4, dm.c2, acc);
+                if (fail) run_cold(fail, 4, C::W1, M, M);
+            }
+        }
+#pragma unroll 1
+        for (int k = 1; k < G::E * G::E; ++k) {
+            const int kk = (k + (G::E * G::E) / 2) % (G::E * G::E);
+            const int tz = kk / G::E, ty = kk % G::E;   // offset + M
+            const float2 *bRow = ((ty & 1) ? sBO : sBE) + (tz * G::NPE + l + (ty >> 1)) * G::PB2 + x0;
+            unsigned fail = pair_pass<RZ, C::W0, false, AP, BP>(aRow, bRow, dm.c2, acc);
+            if (fail) run_cold(fail, 0, C::W0, ty, tz);
+            if constexpr (C::W1 > 0) {
+                fail = pair_pass<RZ, C::W1, false, AP, BP>(aRow, bRow + 4, dm.c2, acc);
+                if (fail) run_cold(fail, 4, C::W1, ty, tz);
+            }
+        }
+
+        // epilogue: rows 2l (.x) and 2l+1 (.y); tile rows 1..30 are outputs
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int r = 2 * l + e, y = Y0 - 1 + r;
+            if (r >= 1 && r <= kPairRowsOut && y < dm.Y && col_ok) {
+                const size_t base0 = (size_t)ph * V + ((size_t)Z0 * dm.Y + y) * dm.X + X0 + x0;
+#pragma unroll
+                for (int o = 0; o < RZ; ++o) {
+                    if (Z0 + o < dm.z_end) {
+                        float nlm[2];
+#pragma unroll
+                        for (int i = 0; i < 2; ++i)
+                            nlm[i] = e ? __fdividef(acc[o].n[i].y, acc[o].z[i].y) : __fdividef(acc[o].n[i].x, acc[o].z[i].x);
+                        float *dst = f_out + base0 + o * zstride;
+                        if (s == 0) {
+                            // park NLM- in f_out; the same thread reads it back after the second direction
+                            if (vec_ok) {
+                                *reinterpret_cast<float2 *>(dst) = make_float2(nlm[0], nlm[1]);
+                            } else {
+                                dst[0] = nlm[0];
+                                if (X0 + x0 + 1 < dm.X) dst[1] = nlm[1];
+                            }
+                        } else {
+                            // a5: Jacobi combine (Eq. 8)
+                            const float *gp = g + base0 + o * zstride;
+                            if (vec_ok) {
+                                const float2 gv = __ldg(reinterpret_cast<const float2 *>(gp));
+                                const float2 pv = *reinterpret_cast<const float2 *>(dst);
+                                *reinterpret_cast<float2 *>(dst) =
+                                    make_float2(fmaf(dm.a_g, gv.x, dm.a_n * (pv.x + nlm[0])),
+                                                fmaf(dm.a_g, gv.y, dm.a_n * (pv.y + nlm[1])));
+                            } else {
+                                dst[0] = fmaf(dm.a_g, __ldg(gp), dm.a_n * (dst[0] + nlm[0]));
+                                if (X0 + x0 + 1 < dm.X) dst[1] = fmaf(dm.a_g, __ldg(gp + 1), dm.a_n * (dst[1] + nlm[1]));
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+inline bool pair_supported(const tnlm_params &p)
+{
+    return p.patch_radius == 1 && p.search_radius >= 1 && p.search_radius <= 4;
+}
+inline const char *pair_name(const tnlm_params &p)
+{
+    switch (p.search_radius) {
+        case 1: return "tnlm_pair_kernel<M=1>";
+        case 2: return "tnlm_pair_kernel<M=2>";
+        case 3: return "tnlm_pair_kernel<M=3>";
+        default: return "tnlm_pair_kernel<M=4>";
+    }
+}
+
+template <int M, int RZ, int TX>
+cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, float *f_out, cudaStream_t st)
+{
+    using G = PairGeom<M, RZ, TX>;
+    static_assert(G::BYTES <= 227 * 1024, "pair kernel tile does not fit in shared memory");
+    static bool configured = false;   // per template instance; the attribute is idempotent
+    cudaError_t e;
+    if (!configured) {
+        e = cudaFuncSetAttribute(tnlm_pair_kernel<M, RZ, TX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int tiles_x = (dm.X + TX - 1) / TX;
+    const int tiles_y = (dm.Y + kPairRowsOut - 1) / kPairRowsOut;
+    const int tiles_z = (dm.z_end - dm.z_begin + RZ - 1) / RZ;
+    const long long blocks = (long long)tiles_x * tiles_y * tiles_z * dm.P;
+    if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
+    tnlm_pair_kernel<M, RZ, TX><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
+    return cudaGetLastError();
+}
+
+// ref must be f (TNLM-E); the caller falls back to the generic kernel otherwise.
+inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float *f, const float *g, const float *ref,
+                               float *f_out, cudaStream_t st)
+{
+    if (ref != f) return cudaErrorNotSupported;
+    switch (p.search_radius) {
+        case 1: return launch_pair_t<1, 8, 16>(dm, f, g, f_out, st);
+        case 2: {
+            static const int rz = tiled_env("TNLM_PAIR_RZ", 4);   // tuning knob for experiments
+            if (rz == 6) return launch_pair_t<2, 6, 16>(dm, f, g, f_out, st);
+            if (rz == 4) return launch_pair_t<2, 4, 16>(dm, f, g, f_out, st);
+            return launch_pair_t<2, 8, 16>(dm, f, g, f_out, st);
+        }
+        case 3: return launch_pair_t<3, 6, 32>(dm, f, g, f_out, st);
+        case 4: return launch_pair_t<4, 4, 32>(dm, f, g, f_out, st);
+        default: return cudaErrorNotSupported;
+    }
+}
+
+}  // namespace tnlm

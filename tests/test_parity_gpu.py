@@ -26,6 +26,7 @@ def variants(T, p):
     out = [T.VARIANT_GENERIC]
     if T.kernel_name(p) != "jacobi_generic_kernel":
         out.append(T.VARIANT_TILED)
+        out.append(T.VARIANT_PAIRED)
     return out
 
 
