@@ -20,7 +20,7 @@
 //   per (ty,tz) = a "pass": march the RZ+2 planes; per plane, for W consecutive tx at once
 //       a1  d = b + (-a)                                      FADD2, operands straight from LDS.128 windows
 //       a2x 3-tap x-sum of squares; the two outputs share the middle pair    FMUL2 + 3 FFMA2 per 2 outputs
-//       a2z 3-tap z-sum from a two-plane register ring                       2 FADD2
+//       a2z 3-tap z-sum from a two-plane register ring; even/odd outputs share a pair sum   1.5 FADD2
 //       a2y S.lo + S.hi (own two rows) + one row from the lane above / below  1 FADD + 2 SHFL + 1 FADD2
 //       a3  u = ex2(bias - c2*D)                                              FFMA2 + 2 MUFU.EX2
 //       a4  Z += u, N += u * f_j(x+t)                                         FADD2 + FFMA2
@@ -123,7 +123,14 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                 float2 D[W];
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    const float2 S = add2(add2(ring0[q][i], ring1[q][i]), X[q][i]);       // a2z
+                    // a2z: outputs (o, o+1), o even, share X[o+1] + X[o+2]: 3 adds per 2 outputs
+                    float2 S;
+                    if ((p & 1) == 0) {
+                        ring1[q][i] = add2(ring1[q][i], X[q][i]);    // X[o+1] + X[o+2]
+                        S = add2(ring0[q][i], ring1[q][i]);
+                    } else {
+                        S = add2(ring0[q][i], X[q][i]);              // ring0 holds the shared pair sum
+                    }
                     const float own = S.x + S.y;                                          // a2y
                     const float up = __shfl_up_sync(0xffffffffu, S.y, 1);                 // row 2l-1
                     const float dn = __shfl_down_sync(0xffffffffu, S.x, 1);               // row 2l+2
@@ -135,10 +142,11 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                     for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
                     ac.b[i] = make_float2(c2 * dmin.x, c2 * dmin.y);
                 }
+                const float2 bias = ac.b[i];
                 float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    const float2 arg = fma2(D[q], nc2, ac.b[i]);                          // a3
+                    const float2 arg = fma2(D[q], nc2, bias);                             // a3
                     const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
                     zp = add2(zp, u);                                                     // a4
                     np = fma2(u, bprev[i + 1 + q], np);
@@ -154,6 +162,7 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                 }
             }
         }
+        // ring state after plane p: p < 2 or p odd -> (X[p-1], X[p]); p even -> (X[p-1] + X[p], X[p])
 #pragma unroll
         for (int q = 0; q < W; ++q)
 #pragma unroll
@@ -228,7 +237,7 @@ __device__ __noinline__ void pair_cold(float *accl, unsigned fail, const float *
 //   dstE pair r/2 (half r&1); dstO (optional) pair (r-1)/2 (half (r-1)&1) for r >= 1
 // The (r, c) of a thread's k-th element is the same in every plane, so its global offset inside a
 // plane and its shared-memory offsets are tabulated once; the plane loop is then LDG + STS only,
-// two planes (2K loads) in flight per thread.
+// four planes (4K loads) in flight per thread.
 template <int PITCH2, int ROWS, int COLS, int PLANES, int NP, bool ODD, bool NEGATE, int NT>
 __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__restrict__ dstO,
                                             const float *__restrict__ src, const int zo, const int yo, const int xo,
@@ -236,6 +245,7 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
 {
     constexpr int K = (ROWS * COLS + NT - 1) / NT;
     constexpr int PLANE_F = NP * PITCH2 * 2;   // floats per shared-memory plane
+    constexpr int PF = 4;                      // planes in flight
     int goff[K], eoff[K], ooff[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
@@ -250,16 +260,16 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
     }
     const size_t plane = (size_t)dm.Y * dm.X;
 #pragma unroll 1
-    for (int pz = 0; pz < PLANES; pz += 2) {
-        float v[2][K];
+    for (int pz = 0; pz < PLANES; pz += PF) {
+        float v[PF][K];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
+        for (int h = 0; h < PF; ++h) {
             const float *sp = src + (size_t)clampi(zo + min(pz + h, PLANES - 1), dm.Z) * plane;
 #pragma unroll
             for (int k = 0; k < K; ++k) v[h][k] = __ldg(sp + goff[k]);
         }
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
+        for (int h = 0; h < PF; ++h) {
             if (pz + h < PLANES) {
                 float *dE = dstE + (pz + h) * PLANE_F;
                 float *dO = dstO + (pz + h) * PLANE_F;
@@ -275,7 +285,7 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
 }
 
 template <int M, int RZ, int TX>
-__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, (PairGeom<M, RZ, TX>::NT <= 128) ? 2 : 1)
+__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, (PairGeom<M, RZ, TX>::NT <= 192) ? 2 : 1)
 tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float *f_out, const Dims dm,
                  const int tiles_x, const int tiles_y, const int tiles_z)
 {
@@ -292,7 +302,9 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
     const int by = t % tiles_y; t /= tiles_y;
     const int bz = t % tiles_z; t /= tiles_z;
     const int ph = t;
-    const int X0 = bx * TX, Y0 = by * kPairRowsOut, Z0 = dm.z_begin + bz * RZ;
+    // z-tiles are aligned to absolute multiples of RZ, so a voxel is computed at the same place of a tile
+    // (same rounding) whatever output slab [z_begin, z_end) the call covers
+    const int X0 = bx * TX, Y0 = by * kPairRowsOut, Z0 = (dm.z_begin / RZ + bz) * RZ;
     const size_t V = (size_t)dm.Z * dm.Y * dm.X;
     const int tid = threadIdx.x;
     const int l = tid & 15;            // row pair: tile rows 2l, 2l+1
@@ -369,44 +381,74 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
         }
 
         // epilogue: rows 2l (.x) and 2l+1 (.y); tile rows 1..30 are outputs
+        bool row_ok[2];
+        size_t base0[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int r = 2 * l + e, y = Y0 - 1 + r;
-            if (r >= 1 && r <= kPairRowsOut && y < dm.Y && col_ok) {
-                const size_t base0 = (size_t)ph * V + ((size_t)Z0 * dm.Y + y) * dm.X + X0 + x0;
+            row_ok[e] = r >= 1 && r <= kPairRowsOut && y < dm.Y && col_ok;
+            base0[e] = (size_t)ph * V + ((size_t)Z0 * dm.Y + min(y, dm.Y - 1)) * dm.X + X0 + x0;
+        }
+        if (s == 0) {
+            // park NLM- in f_out; the same thread reads it back after the second direction
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
 #pragma unroll
                 for (int o = 0; o < RZ; ++o) {
-                    if (Z0 + o < dm.z_end) {
-                        float nlm[2];
-#pragma unroll
-                        for (int i = 0; i < 2; ++i)
-                            nlm[i] = e ? __fdividef(acc[o].n[i].y, acc[o].z[i].y) : __fdividef(acc[o].n[i].x, acc[o].z[i].x);
-                        float *dst = f_out + base0 + o * zstride;
-                        if (s == 0) {
-                            // park NLM- in f_out; the same thread reads it back after the second direction
-                            if (vec_ok) {
-                                *reinterpret_cast<float2 *>(dst) = make_float2(nlm[0], nlm[1]);
-                            } else {
-                                dst[0] = nlm[0];
-                                if (X0 + x0 + 1 < dm.X) dst[1] = nlm[1];
-                            }
+                    if (row_ok[e] && Z0 + o >= dm.z_begin && Z0 + o < dm.z_end) {
+                        const float n0 = e ? __fdividef(acc[o].n[0].y, acc[o].z[0].y) : __fdividef(acc[o].n[0].x, acc[o].z[0].x);
+                        const float n1 = e ? __fdividef(acc[o].n[1].y, acc[o].z[1].y) : __fdividef(acc[o].n[1].x, acc[o].z[1].x);
+                        float *dst = f_out + base0[e] + o * zstride;
+                        if (vec_ok) {
+                            *reinterpret_cast<float2 *>(dst) = make_float2(n0, n1);
                         } else {
-                            // a5: Jacobi combine (Eq. 8)
-                            const float *gp = g + base0 + o * zstride;
-                            if (vec_ok) {
-                                const float2 gv = __ldg(reinterpret_cast<const float2 *>(gp));
-                                const float2 pv = *reinterpret_cast<const float2 *>(dst);
-                                *reinterpret_cast<float2 *>(dst) =
-                                    make_float2(fmaf(dm.a_g, gv.x, dm.a_n * (pv.x + nlm[0])),
-                                                fmaf(dm.a_g, gv.y, dm.a_n * (pv.y + nlm[1])));
-                            } else {
-                                dst[0] = fmaf(dm.a_g, __ldg(gp), dm.a_n * (dst[0] + nlm[0]));
-                                if (X0 + x0 + 1 < dm.X) dst[1] = fmaf(dm.a_g, __ldg(gp + 1), dm.a_n * (dst[1] + nlm[1]));
+                            dst[0] = n0;
+                            if (X0 + x0 + 1 < dm.X) dst[1] = n1;
+                        }
+                    }
+                }
+        } else {
+            // a5: Jacobi combine (Eq. 8); all loads are issued before the first dependent use
+            float2 gv[2][RZ], pv[2][RZ];
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int o = 0; o < RZ; ++o) {
+                    gv[e][o] = pv[e][o] = make_float2(0.f, 0.f);
+                    if (row_ok[e] && Z0 + o >= dm.z_begin && Z0 + o < dm.z_end) {
+                        const float *gp = g + base0[e] + o * zstride;
+                        const float *pp = f_out + base0[e] + o * zstride;
+                        if (vec_ok) {
+                            gv[e][o] = __ldg(reinterpret_cast<const float2 *>(gp));
+                            pv[e][o] = *reinterpret_cast<const float2 *>(pp);
+                        } else {
+                            gv[e][o].x = __ldg(gp);
+                            pv[e][o].x = pp[0];
+                            if (X0 + x0 + 1 < dm.X) {
+                                gv[e][o].y = __ldg(gp + 1);
+                                pv[e][o].y = pp[1];
                             }
                         }
                     }
                 }
-            }
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int o = 0; o < RZ; ++o) {
+                    if (row_ok[e] && Z0 + o >= dm.z_begin && Z0 + o < dm.z_end) {
+                        const float n0 = e ? __fdividef(acc[o].n[0].y, acc[o].z[0].y) : __fdividef(acc[o].n[0].x, acc[o].z[0].x);
+                        const float n1 = e ? __fdividef(acc[o].n[1].y, acc[o].z[1].y) : __fdividef(acc[o].n[1].x, acc[o].z[1].x);
+                        const float r0 = fmaf(dm.a_g, gv[e][o].x, dm.a_n * (pv[e][o].x + n0));
+                        const float r1 = fmaf(dm.a_g, gv[e][o].y, dm.a_n * (pv[e][o].y + n1));
+                        float *dst = f_out + base0[e] + o * zstride;
+                        if (vec_ok) {
+                            *reinterpret_cast<float2 *>(dst) = make_float2(r0, r1);
+                        } else {
+                            dst[0] = r0;
+                            if (X0 + x0 + 1 < dm.X) dst[1] = r1;
+                        }
+                    }
+                }
         }
     }
 }
@@ -440,7 +482,7 @@ cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, float 
     }
     const int tiles_x = (dm.X + TX - 1) / TX;
     const int tiles_y = (dm.Y + kPairRowsOut - 1) / kPairRowsOut;
-    const int tiles_z = (dm.z_end - dm.z_begin + RZ - 1) / RZ;
+    const int tiles_z = (dm.z_end + RZ - 1) / RZ - dm.z_begin / RZ;   // tiles aligned to multiples of RZ
     const long long blocks = (long long)tiles_x * tiles_y * tiles_z * dm.P;
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
     tnlm_pair_kernel<M, RZ, TX><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
@@ -455,7 +497,9 @@ inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float
     switch (p.search_radius) {
         case 1: return launch_pair_t<1, 8, 16>(dm, f, g, f_out, st);
         case 2: {
-            static const int rz = tiled_env("TNLM_PAIR_RZ", 4);   // tuning knob for experiments
+            static const int rz = tiled_env("TNLM_PAIR_RZ", 6);   // tuning knob for experiments
+            static const int tx = tiled_env("TNLM_PAIR_TX", 16);
+            if (tx == 24) return launch_pair_t<2, 4, 24>(dm, f, g, f_out, st);
             if (rz == 6) return launch_pair_t<2, 6, 16>(dm, f, g, f_out, st);
             if (rz == 4) return launch_pair_t<2, 4, 16>(dm, f, g, f_out, st);
             return launch_pair_t<2, 8, 16>(dm, f, g, f_out, st);
