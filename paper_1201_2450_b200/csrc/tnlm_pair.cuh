@@ -26,14 +26,16 @@
 //       a4  Z += u, N += u * f_j(x+t)                                         FADD2 + FFMA2
 //   epilogue    = NLM of the first direction is parked in f_out (same thread reads it back), then
 //                 a5: f_out = mu/(2+mu) g + (NLM- + NLM+)/(2+mu)
-// Reference exponent (reading P3: weights relative to the best candidate).  The first pass (zero y/z
-// offset) sets the reference exponent of every output from its best candidate; later passes add their
-// terms optimistically and check the partial normaliser against a 2^100 guard band.  Row pairs whose
-// terms left the band (a candidate > 2^100 times better than the reference: moving high-contrast edges)
-// are not added; the thread re-does them in pair_cold (direct 27-tap distances, re-base, add).  The
-// result equals the shifted softmax up to rounding.
+// Reference exponent (reading P3: weights relative to the best candidate).  Every output keeps a
+// reference exponent b; a pass sums its W terms ex2(b - c2*D) optimistically.  If the partial
+// normaliser stays below 2^100 (no candidate ~2^100 times better than the reference) it is added as
+// it is; otherwise (first use, b = +inf; later only at moving high-contrast edges) nothing is added,
+// the row pair is flagged, and the warp re-does that pass in a careful form that re-bases flagged
+// pairs on min(b, c2*Dmin of the pass) and re-evaluates their terms.  The result equals the shifted
+// softmax up to rounding.
 #pragma once
 #include <cstdlib>
+#include <type_traits>
 
 #include "tnlm_common.cuh"
 #include "tnlm_tiled.cuh"
@@ -72,7 +74,7 @@ template <int M, int RZ, int TX> struct PairGeom {
 
 struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
 
-constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100: Z stays below 2^107 (safe for __fdividef)
+constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100: partial sums up to here are added as they are; Z < 2^107 (safe for __fdividef)
 
 template <int NV>
 __device__ __forceinline__ void load_pairs(const float2 *__restrict__ p, float2 (&dst)[2 * NV])
@@ -88,13 +90,16 @@ __device__ __forceinline__ void load_pairs(const float2 *__restrict__ p, float2 
 // One pass: W consecutive x-offsets at fixed (ty, tz), marching the RZ+2 planes.
 //   aRow: &A2[plane 0][pair l][x0]                 element k <-> x = X0 + x0 - 1 + k   (negated values)
 //   bRow: &B?[plane tz][pair l + ty/2][x0 + q0]    element k + q pairs with a[k] for the q-th offset of the chunk
-// FIRST: the accumulators are empty; the reference exponent of every output is set from the best
-//        candidate of this pass (exact, no guard needed).
-// else : optimistic add; returns a bit mask (bit 2*o + i) of the row pairs whose terms left the guard
-//        band and were NOT added (the caller sends those through pair_cold).
-template <int RZ, int W, bool FIRST, int A_PLANE, int B_PLANE>
+// CAREFUL = false (hot): the W terms of a row pair are summed optimistically relative to its reference
+//   exponents and added if the partial normaliser stayed inside the guard band; otherwise nothing is
+//   added and bit 2*o + i of the returned mask is set.
+// CAREFUL = true: only the row pairs named in `mask` are touched; on a guard failure the pair is
+//   re-based on min(reference, c2*Dmin of the pass), branch-free for its two rows, and the terms are
+//   re-evaluated.  Used for the first pass (reference = +inf) and to re-do a pass that reported failures.
+// Both forms execute the same shuffles, so a warp may run them with different masks per lane.
+template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE>
 __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
-                                              const float c2, AccPair (&acc)[RZ])
+                                              const float c2, AccPair (&acc)[RZ], const unsigned mask)
 {
     constexpr int NVB = (W + 4) / 2;
     const float2 nc2 = make_float2(-c2, -c2);
@@ -136,29 +141,36 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                     const float dn = __shfl_down_sync(0xffffffffu, S.x, 1);               // row 2l+2
                     D[q] = add2(make_float2(up, dn), make_float2(own, own));
                 }
-                if (FIRST) {
-                    float2 dmin = D[0];
+                if (!CAREFUL || ((mask >> (2 * (p - 2) + i)) & 1u)) {
+                    float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
 #pragma unroll
-                    for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
-                    ac.b[i] = make_float2(c2 * dmin.x, c2 * dmin.y);
-                }
-                const float2 bias = ac.b[i];
-                float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
+                    for (int q = 0; q < W; ++q) {
+                        const float2 arg = fma2(D[q], nc2, ac.b[i]);                      // a3
+                        const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
+                        zp = add2(zp, u);                                                 // a4
+                        np = fma2(u, bprev[i + 1 + q], np);
+                    }
+                    if (fmaxf(zp.x, zp.y) <= kPairGuard) {
+                        ac.z[i] = add2(ac.z[i], zp);
+                        ac.n[i] = add2(ac.n[i], np);
+                    } else if (!CAREFUL) {
+                        fail |= 1u << (2 * (p - 2) + i);
+                    } else {
+                        float2 dmin = D[0];
 #pragma unroll
-                for (int q = 0; q < W; ++q) {
-                    const float2 arg = fma2(D[q], nc2, bias);                             // a3
-                    const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
-                    zp = add2(zp, u);                                                     // a4
-                    np = fma2(u, bprev[i + 1 + q], np);
-                }
-                if (FIRST) {
-                    ac.z[i] = zp;
-                    ac.n[i] = np;
-                } else if (fmaxf(zp.x, zp.y) <= kPairGuard) {
-                    ac.z[i] = add2(ac.z[i], zp);
-                    ac.n[i] = add2(ac.n[i], np);
-                } else {
-                    fail |= 1u << (2 * (p - 2) + i);
+                        for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
+                        const float2 nb = make_float2(fminf(c2 * dmin.x, ac.b[i].x), fminf(c2 * dmin.y, ac.b[i].y));
+                        const float2 sc = make_float2(ex2(nb.x - ac.b[i].x), ex2(nb.y - ac.b[i].y));   // 1 if unchanged, 0 on first use
+                        float2 zz = mul2(ac.z[i], sc), nn = mul2(ac.n[i], sc);
+#pragma unroll
+                        for (int q = 0; q < W; ++q) {
+                            const float2 ar = fma2(D[q], nc2, nb);
+                            const float2 u = make_float2(ex2(ar.x), ex2(ar.y));
+                            zz = add2(zz, u);
+                            nn = fma2(u, bprev[i + 1 + q], nn);
+                        }
+                        ac.z[i] = zz; ac.n[i] = nn; ac.b[i] = nb;
+                    }
                 }
             }
         }
@@ -174,62 +186,6 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
         for (int k = 0; k < 2 * NVB; ++k) bprev[k] = b[k];
     }
     return fail;
-}
-
-// Cold path: re-do the W terms of the flagged row pairs (bit 2*o + i of `fail`) with distances taken
-// directly from the tiles, re-basing an output on its best candidate when that beats its reference.
-//   accl: the thread's accumulators, [(2*o + i)*6 + {z.x, z.y, n.x, n.y, b.x, b.y}]
-template <int M, int RZ, int TX>
-__device__ __noinline__ void pair_cold(float *accl, unsigned fail, const float *__restrict__ sA,
-                                       const float *__restrict__ sBE, const int l, const int x0, const int q0,
-                                       const int W, const int ty, const int tz, const float c2)
-{
-    using G = PairGeom<M, RZ, TX>;
-    while (fail) {
-        const int bit = __ffs(fail) - 1;
-        fail &= fail - 1;
-        const int o = bit >> 1, i = bit & 1;
-        float *ac = accl + bit * 6;
-#pragma unroll 1
-        for (int e = 0; e < 2; ++e) {
-            const int r = 2 * l + e;
-            float D[5], v[5];
-            float Dmin = INFINITY;
-#pragma unroll 1
-            for (int q = 0; q < W; ++q) {
-                float acc = 0.f;
-                for (int dz = -1; dz <= 1; ++dz)
-                    for (int dy = -1; dy <= 1; ++dy) {
-                        const int ra = min(max(r + dy, 0), 31), rb = min(max(r + ty + dy, 0), 31 + 2 * M);
-                        const float *pa = sA + (((o + 1 + dz) * G::NPA + (ra >> 1)) * G::PA2 + x0 + i + 1) * 2 + (ra & 1);
-                        const float *pb = sBE + (((o + 1 + tz + dz) * G::NPE + (rb >> 1)) * G::PB2 + x0 + i + 1 + q0 + q) * 2 + (rb & 1);
-                        for (int dx = -1; dx <= 1; ++dx) {
-                            const float d = pa[2 * dx] + pb[2 * dx];   // sA holds -ref_i
-                            acc = fmaf(d, d, acc);
-                        }
-                    }
-                const int rb = r + ty;
-                v[q] = sBE[(((o + 1 + tz) * G::NPE + (rb >> 1)) * G::PB2 + x0 + i + 1 + q0 + q) * 2 + (rb & 1)];
-                D[q] = acc;
-                Dmin = fminf(Dmin, acc);
-            }
-            float Z = ac[e], N = ac[2 + e], bias = ac[4 + e];
-            const float nb = c2 * Dmin;
-            if (nb < bias) {   // a better candidate than the reference: re-base
-                const float sc = ex2(nb - bias);
-                Z *= sc;
-                N *= sc;
-                bias = nb;
-            }
-#pragma unroll 1
-            for (int q = 0; q < W; ++q) {
-                const float u = ex2(fmaf(-c2, D[q], bias));
-                Z += u;
-                N = fmaf(u, v[q], N);
-            }
-            ac[e] = Z; ac[2 + e] = N; ac[4 + e] = bias;
-        }
-    }
 }
 
 // Stage a clamped halo tile into row-pair layout(s):
@@ -328,56 +284,34 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
             X0 - 1 - M, dm, tid);
         __syncthreads();
 
-        AccPair acc[RZ];   // fully written by the first pass
+        AccPair acc[RZ];
+#pragma unroll
+        for (int o = 0; o < RZ; ++o)
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                acc[o].z[i] = make_float2(0.f, 0.f);
+                acc[o].n[i] = make_float2(0.f, 0.f);
+                acc[o].b[i] = make_float2(INFINITY, INFINITY);   // first use takes the re-base path
+            }
         const float2 *aRow = sA + l * G::PA2 + x0;
         static_assert(G::NPE == G::NPO, "BE and BO share one plane stride");
-
-        // the thread's accumulators take a round trip through local memory around the (rare) cold path
-        auto run_cold = [&](unsigned fail, int q0, int W, int ty, int tz) {
-            float accl[RZ * 12];
-#pragma unroll
-            for (int o = 0; o < RZ; ++o)
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    float *a6 = accl + (2 * o + i) * 6;
-                    a6[0] = acc[o].z[i].x; a6[1] = acc[o].z[i].y;
-                    a6[2] = acc[o].n[i].x; a6[3] = acc[o].n[i].y;
-                    a6[4] = acc[o].b[i].x; a6[5] = acc[o].b[i].y;
-                }
-            pair_cold<M, RZ, TX>(accl, fail, reinterpret_cast<const float *>(sA), reinterpret_cast<const float *>(sBE), l,
-                                 x0, q0, W, ty, tz, dm.c2);
-#pragma unroll
-            for (int o = 0; o < RZ; ++o)
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    const float *a6 = accl + (2 * o + i) * 6;
-                    acc[o].z[i] = make_float2(a6[0], a6[1]);
-                    acc[o].n[i] = make_float2(a6[2], a6[3]);
-                    acc[o].b[i] = make_float2(a6[4], a6[5]);
-                }
+        // a chunk of a pass: hot form first; if any lane of the warp reports guard failures, the whole
+        // warp re-does the chunk in the careful form (each lane with its own mask of failed row pairs)
+        auto run_chunk = [&](auto wtag, const float2 *bRow, const bool first) {
+            constexpr int W = decltype(wtag)::value;
+            unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
+            if (!first) fail = pair_pass<RZ, W, false, AP, BP>(aRow, bRow, dm.c2, acc, 0u);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail);
         };
-
-        // first pass: (ty, tz) = zero offset; its first chunk sets every output's reference exponent
-        // (the zero offset is usually the best match, so the cold path stays cold)
-        {
-            const float2 *bRow = ((M & 1) ? sBO : sBE) + (M * G::NPE + l + (M >> 1)) * G::PB2 + x0;
-            pair_pass<RZ, C::W0, true, AP, BP>(aRow, bRow, dm.c2, acc);
-            if constexpr (C::W1 > 0) {
-                const unsigned fail = pair_pass<RZ, C::W1, false, AP, BP>(aRow, bRow + 4, dm.c2, acc);
-                if (fail) run_cold(fail, 4, C::W1, M, M);
-            }
-        }
 #pragma unroll 1
-        for (int k = 1; k < G::E * G::E; ++k) {
+        for (int k = 0; k < G::E * G::E; ++k) {
+            // start with (ty, tz) = (0, 0): the zero offset is usually the best match, so the reference
+            // exponents are set once, in the first pass, and the careful form stays cold afterwards
             const int kk = (k + (G::E * G::E) / 2) % (G::E * G::E);
             const int tz = kk / G::E, ty = kk % G::E;   // offset + M
             const float2 *bRow = ((ty & 1) ? sBO : sBE) + (tz * G::NPE + l + (ty >> 1)) * G::PB2 + x0;
-            unsigned fail = pair_pass<RZ, C::W0, false, AP, BP>(aRow, bRow, dm.c2, acc);
-            if (fail) run_cold(fail, 0, C::W0, ty, tz);
-            if constexpr (C::W1 > 0) {
-                fail = pair_pass<RZ, C::W1, false, AP, BP>(aRow, bRow + 4, dm.c2, acc);
-                if (fail) run_cold(fail, 4, C::W1, ty, tz);
-            }
+            run_chunk(std::integral_constant<int, C::W0>{}, bRow, k == 0);
+            if constexpr (C::W1 > 0) run_chunk(std::integral_constant<int, C::W1>{}, bRow + 4, false);
         }
 
         // epilogue: rows 2l (.x) and 2l+1 (.y); tile rows 1..30 are outputs
@@ -497,14 +431,18 @@ inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float
     switch (p.search_radius) {
         case 1: return launch_pair_t<1, 8, 16>(dm, f, g, f_out, st);
         case 2: {
-            static const int rz = tiled_env("TNLM_PAIR_RZ", 6);   // tuning knob for experiments
+            static const int rz = tiled_env("TNLM_PAIR_RZ", 4);   // tuning knob for experiments
             static const int tx = tiled_env("TNLM_PAIR_TX", 16);
             if (tx == 24) return launch_pair_t<2, 4, 24>(dm, f, g, f_out, st);
             if (rz == 6) return launch_pair_t<2, 6, 16>(dm, f, g, f_out, st);
             if (rz == 4) return launch_pair_t<2, 4, 16>(dm, f, g, f_out, st);
             return launch_pair_t<2, 8, 16>(dm, f, g, f_out, st);
         }
-        case 3: return launch_pair_t<3, 6, 32>(dm, f, g, f_out, st);
+        case 3: {
+            static const int tx = tiled_env("TNLM_PAIR_TX3", 32);
+            if (tx == 16) return launch_pair_t<3, 4, 16>(dm, f, g, f_out, st);
+            return launch_pair_t<3, 6, 32>(dm, f, g, f_out, st);
+        }
         case 4: return launch_pair_t<4, 4, 32>(dm, f, g, f_out, st);
         default: return cudaErrorNotSupported;
     }
