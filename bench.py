@@ -288,10 +288,13 @@ def main():
     achieved = cfg.updates_per_sweep * A / (launch_ms * 1e-3)
     peak = sms * SM_LANES * peaks["sm_max_mhz"] * 1e6
     alg_bytes = 3 * g.numel() * 4                      # read f, read g, write f_out
-    traffic = None
+    traffic = None          # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            traffic = json.load(fh).get(T.kernel_name(p))
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == T.kernel_name(p) and cfg.name == "config3":
+                    traffic = int(row["dram_bytes_per_launch"])
     except Exception:
         pass
     roofline = {
