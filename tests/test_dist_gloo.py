@@ -1,0 +1,111 @@
+"""The multi-process plumbing (paper_1201_2450_b200/dist.py) on CPU: world_size 2, gloo, 127.0.0.1.
+
+The z-slab partition of one stack: every rank owns a contiguous slab of planes
+of every phase and needs the M+d planes next to it from its neighbours before each sweep
+(Eq. 8 reads f_{i+-1} inside the window of PAPER.md:223).  The tests check that
+  * the slabs tile the volume,
+  * exchange_halos delivers exactly the planes a sweep reads (everything else in the rank's copy is
+    poisoned with NaN, so a missing plane shows up in the result),
+  * two sweeps computed slab-wise on 2 ranks (oracle arithmetic, halo exchange in between) equal two
+    sweeps of the whole stack bit for bit,
+  * the max / sum reductions that bench.py uses for timing.
+"""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, shape, d, M, h, mu, n_sweeps, out_dir):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    from oracle import tnlm_oracle as O
+    from tnlm_inputs import random_stack
+
+    info = D.init("gloo")
+    assert info.world == world and info.rank == rank
+    P, Z, Y, X = shape
+    g_full = random_stack(shape, 7)
+    a, b = D.z_slab(Z, rank, world)
+
+    # this rank's copy: its own slab is valid, everything else is poison
+    f = np.full(shape, np.nan, dtype=np.float32)
+    f[:, a:b] = g_full[:, a:b]
+    plane = Y * X
+    own = (np.arange(P)[:, None] * Z * plane + (np.arange(a * plane, b * plane))[None, :]).reshape(-1).astype(np.int64)
+    for _ in range(n_sweeps):
+        ft = torch.from_numpy(f)
+        D.exchange_halos(info, ft, M + d)
+        lo, hi = max(a - (M + d), 0), min(b + (M + d), Z)
+        assert np.isfinite(f[:, lo:hi]).all(), "a plane inside the halo was not delivered"
+        # the oracle clamps coordinates to the volume: give it finite values outside the halo that a
+        # correct sweep never reads for this slab... it does not read them, so any value works
+        work = np.where(np.isfinite(f), f, np.float32(1e30))
+        new = O.jacobi_step_at(work, g_full, d, M, np.float32(h), np.float32(mu), own)
+        f = np.full(shape, np.nan, dtype=np.float32)
+        f.reshape(-1)[own] = new
+    np.save(os.path.join(out_dir, f"slab{rank}.npy"), f[:, a:b])
+
+    t = D.max_over_ranks(info, float(rank + 1))
+    s = D.sum_over_ranks(info, float(rank + 1))
+    assert t == float(world) and s == world * (world + 1) / 2
+    D.barrier(info)
+    D.finalize(info)
+
+
+def test_z_slabs_tile_the_volume():
+    from paper_1201_2450_b200 import dist as D
+    for n in (1, 5, 16, 100, 128):
+        for world in (1, 2, 3, 8):
+            slabs = [D.z_slab(n, r, world) for r in range(world)]
+            assert slabs[0][0] == 0 and slabs[-1][1] == n
+            assert all(slabs[i][1] == slabs[i + 1][0] for i in range(world - 1))
+            sizes = [b - a for a, b in slabs]
+            assert max(sizes) - min(sizes) <= 1
+
+
+@pytest.mark.parametrize("d,M,Z", [(1, 2, 9), (1, 1, 4), (2, 1, 7)])
+def test_two_rank_slab_sweeps_equal_the_full_sweeps(tmp_path, oracle, d, M, Z):
+    import torch.multiprocessing as mp
+    shape = (3, Z, 6, 7)
+    h, mu, n_sweeps, world = 0.3, 0.7, 2, 2
+    port = _free_port()
+    mp.spawn(_worker, args=(world, port, shape, d, M, h, mu, n_sweeps, str(tmp_path)), nprocs=world, join=True)
+
+    from tnlm_inputs import random_stack
+    from paper_1201_2450_b200 import dist as D
+    g = random_stack(shape, 7)
+    want = g
+    for _ in range(n_sweeps):
+        want = oracle.jacobi_step(want, g, d, M, np.float32(h), np.float32(mu))
+    got = np.concatenate([np.load(tmp_path / f"slab{r}.npy") for r in range(world)], axis=1)
+    assert got.shape == want.shape
+    assert np.array_equal(got, want), "slab-wise sweeps with halo exchange differ from the full sweeps"
+
+
+def test_single_process_is_a_no_op():
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"):
+        os.environ.pop(k, None)
+    info = D.init("gloo")
+    assert not info.distributed
+    x = torch.arange(24.0).reshape(1, 4, 2, 3)
+    assert D.exchange_halos(info, x, 2) is x
+    assert D.max_over_ranks(info, 3.5) == 3.5 and D.sum_over_ranks(info, 3.5) == 3.5
+    D.barrier(info)
+    D.finalize(info)

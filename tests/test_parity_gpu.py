@@ -102,6 +102,47 @@ def test_edge_cases_one_sweep(T, oracle, shape, d, M, h, mu):
         assert_parity(got, want, 1.0, f"edge {shape} d={d} M={M} variant {v}")
 
 
+def moving_block_stack(shape, shift, seed):
+    """A bright block (0.6 on 0.1) that moves `shift` voxels per phase along z, y and x, plus weak noise:
+    at the block faces the zero offset is a bad match and a shifted candidate is better by far more
+    than 2^100 (small h), so the reference exponent set in the first pass must be re-based later."""
+    P, Z, Y, X = shape
+    rng = np.random.default_rng(seed)
+    out = np.full(shape, 0.1, dtype=np.float64)
+    for ph in range(P):
+        z0, y0, x0 = Z // 4 + shift * ph, Y // 4 + shift * ph, X // 4 + shift * ph
+        out[ph, z0:z0 + Z // 3, y0:y0 + Y // 3, x0:x0 + X // 3] = 0.6
+    out += 0.01 * rng.standard_normal(shape)
+    return out.astype(np.float32)
+
+
+@pytest.mark.parametrize("M,shape", [(1, (3, 13, 33, 21)), (2, (3, 11, 35, 37)), (3, (3, 10, 31, 19)), (4, (2, 9, 30, 18))])
+def test_moving_edges_rebase_path(T, oracle, M, shape):
+    g = moving_block_stack(shape, min(M, 2), 11 + M)
+    h, mu = 0.05, 0.5   # c2*D ~ 650 at a mismatched block face: far outside the 2^100 guard band, still fp32-resolvable
+    p = T.TnlmParams.make(shape, 1, M, h, mu)
+    want = oracle.enhance(g, 1, M, np.float32(h), np.float32(mu), 2)
+    for v in variants(T, p):
+        got = T.tnlm_enhance(p, dev(g), 2, variant=v).cpu().numpy()
+        assert_parity(got, want, dynamic_range(g), f"moving block M={M} variant {v}")
+
+
+RAGGED = [(2, 7, 29, 15), (2, 5, 30, 16), (2, 4, 31, 17), (2, 13, 61, 47), (3, 6, 1, 50), (3, 1, 64, 2)]
+
+
+@pytest.mark.parametrize("shape", RAGGED)
+def test_ragged_tiles_one_sweep(T, oracle, shape):
+    """Extents around the tile sizes of the sweep kernels (30 output rows, 16/32 columns, RZ planes; odd nx
+    takes the scalar epilogue)."""
+    f, g = random_stack(shape, 21), random_stack(shape, 22)
+    for M in (1, 2):
+        p = T.TnlmParams.make(shape, 1, M, 0.25, 0.5)
+        want = oracle.jacobi_step(f, g, 1, M, np.float32(0.25), np.float32(0.5))
+        for v in variants(T, p):
+            got = T.tnlm_jacobi_step(p, dev(f), dev(g), variant=v).cpu().numpy()
+            assert_parity(got, want, 1.0, f"ragged {shape} M={M} variant {v}")
+
+
 def test_separate_ref_stack(T, oracle):
     """TNLM-R usage: weights from ref = g^(k), averages of f."""
     shape = (3, 9, 20, 41)
