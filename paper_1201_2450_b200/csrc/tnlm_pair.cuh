@@ -9,8 +9,9 @@
 // One CTA = one (phase i, TX-wide x-tile, 30-row y-group, RZ-plane z-slab), both neighbour phases in turn
 // (Eq. 8).  Shared memory holds float2 row-pair tiles:
 //   A2 [RZ+2   ][16  ][PA2]   -ref_i, pair k = tile rows (2k, 2k+1), halo d = 1 (stored negated: a1 is an add)
-//   BE [RZ+2+2M][16+M][PB2]    ref_j, pair k = tile rows (2k,   2k+1)   used when the y-offset is even
-//   BO [RZ+2+2M][16+M][PB2]    ref_j, pair k = tile rows (2k+1, 2k+2)   used when the y-offset is odd
+//   B  [RZ+2+2M][31+2M][PB2]   ref_j, halo 1+M; each plane holds two copies of its rows:
+//        BE = pairs 0..15+M,  pair k = tile rows (2k,   2k+1)   used when the y-offset is even
+//        BO = pairs 16+M..,   pair k = tile rows (2k+1, 2k+2)   used when the y-offset is odd
 // (clamp-to-edge applied while staging: reading P4).  The second copy of B keeps the operand of every
 // packed op an aligned register pair for any y-offset.
 //
@@ -66,10 +67,11 @@ template <int M, int RZ, int TX> struct PairGeom {
     static constexpr int BREAD = cmax(TX - 2 + 2 * NVB0, C::W1 ? TX - 2 + 4 + 2 * NVB1 : 0);   // columns a window may touch
     static constexpr int PA2 = pitch2(ACOLS);
     static constexpr int PB2 = pitch2(cmax(BCOLS, BREAD));
-    static constexpr int NPA = 16, NPE = 16 + M, NPO = 16 + M;     // row pairs per plane (BO padded: same plane stride as BE)
+    static constexpr int NPA = 16, NPE = 16 + M, NPO = 15 + M;     // row pairs per plane
+    static constexpr int NPB = NPE + NPO;                          // a B plane = its BE pairs, then its BO pairs
     static constexpr int NAP = RZ + 2, NBP = RZ + 2 + 2 * M;       // planes
-    static constexpr int A_F2 = NAP * NPA * PA2, BE_F2 = NBP * NPE * PB2, BO_F2 = NBP * NPO * PB2;
-    static constexpr size_t BYTES = (size_t)(A_F2 + BE_F2 + BO_F2) * sizeof(float2);
+    static constexpr int A_F2 = NAP * NPA * PA2, B_F2 = NBP * NPB * PB2;
+    static constexpr size_t BYTES = (size_t)(A_F2 + B_F2) * sizeof(float2);
 };
 
 struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
@@ -194,13 +196,14 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
 // The (r, c) of a thread's k-th element is the same in every plane, so its global offset inside a
 // plane and its shared-memory offsets are tabulated once; the plane loop is then LDG + STS only,
 // four planes (4K loads) in flight per thread.
-template <int PITCH2, int ROWS, int COLS, int PLANES, int NP, bool ODD, bool NEGATE, int NT>
+template <int PITCH2, int ROWS, int COLS, int PLANES, int NP, int NPO, bool NEGATE, int NT>
 __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__restrict__ dstO,
                                             const float *__restrict__ src, const int zo, const int yo, const int xo,
                                             const Dims &dm, const int tid)
 {
     constexpr int K = (ROWS * COLS + NT - 1) / NT;
-    constexpr int PLANE_F = NP * PITCH2 * 2;   // floats per shared-memory plane
+    constexpr bool ODD = NPO > 0;
+    constexpr int PLANE_F = (NP + NPO) * PITCH2 * 2;   // floats per shared-memory plane (even pairs, then odd pairs)
     constexpr int PF = 4;                      // planes in flight
     int goff[K], eoff[K], ooff[K];
 #pragma unroll
@@ -211,7 +214,7 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
         goff[k] = clampi(yo + r, dm.Y) * dm.X + clampi(xo + c, dm.X);
         eoff[k] = ok ? (((r >> 1) * PITCH2 + c) * 2 + (r & 1)) : -1;
         const int ro = r - 1;
-        ooff[k] = (ok && ro >= 0 && (ro >> 1) < NP) ? (((ro >> 1) * PITCH2 + c) * 2 + (ro & 1)) : -1;
+        ooff[k] = (ok && ro >= 0 && (ro >> 1) < NPO) ? (((ro >> 1) * PITCH2 + c) * 2 + (ro & 1)) : -1;
         if (!ok) goff[k] = 0;
     }
     const size_t plane = (size_t)dm.Y * dm.X;
@@ -240,18 +243,18 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
     }
 }
 
-template <int M, int RZ, int TX>
-__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, (PairGeom<M, RZ, TX>::NT <= 192) ? 2 : 1)
+template <int M, int RZ, int TX, int NCTA>
+__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, NCTA)
 tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float *f_out, const Dims dm,
                  const int tiles_x, const int tiles_y, const int tiles_z)
 {
     using G = PairGeom<M, RZ, TX>;
     using C = Chunks<M>;
-    constexpr int AP = G::NPA * G::PA2, BP = G::NPE * G::PB2;   // plane strides (float2)
+    constexpr int AP = G::NPA * G::PA2, BP = G::NPB * G::PB2;   // plane strides (float2)
     extern __shared__ __align__(16) float smem[];
     float2 *sA = reinterpret_cast<float2 *>(smem);
     float2 *sBE = sA + G::A_F2;
-    float2 *sBO = sBE + G::BE_F2;
+    float2 *sBO = sBE + G::NPE * G::PB2;   // odd pairs of plane 0
 
     int t = blockIdx.x;
     const int bx = t % tiles_x; t /= tiles_x;
@@ -267,7 +270,7 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
     const int x0 = 2 * (tid >> 4);     // first x of the run, tile relative
 
     // -ref_i tile (halo 1): rows <-> y = Y0-1+r, cols <-> x = X0-1+c, planes <-> z = Z0-1+pz
-    stage_pairs<G::PA2, 32, G::ACOLS, G::NAP, G::NPA, false, true, G::NT>(
+    stage_pairs<G::PA2, 32, G::ACOLS, G::NAP, G::NPA, 0, true, G::NT>(
         reinterpret_cast<float *>(sA), nullptr, f + (size_t)ph * V, Z0 - 1, Y0 - 1, X0 - 1, dm, tid);
 
     const size_t zstride = (size_t)dm.Y * dm.X;
@@ -279,7 +282,7 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
         const int j = (ph + (s ? 1 : dm.P - 1)) % dm.P;
         __syncthreads();   // everyone is done with the previous B tiles
         // f_j tiles (halo 1+M): rows <-> y = Y0-1-M+r, cols <-> x = X0-1-M+c, planes <-> z = Z0-1-M+pz
-        stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NBP, G::NPE, true, false, G::NT>(
+        stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NBP, G::NPE, G::NPO, false, G::NT>(
             reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), f + (size_t)j * V, Z0 - 1 - M, Y0 - 1 - M,
             X0 - 1 - M, dm, tid);
         __syncthreads();
@@ -294,7 +297,6 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
                 acc[o].b[i] = make_float2(INFINITY, INFINITY);   // first use takes the re-base path
             }
         const float2 *aRow = sA + l * G::PA2 + x0;
-        static_assert(G::NPE == G::NPO, "BE and BO share one plane stride");
         // a chunk of a pass: hot form first; if any lane of the warp reports guard failures, the whole
         // warp re-does the chunk in the careful form (each lane with its own mask of failed row pairs)
         auto run_chunk = [&](auto wtag, const float2 *bRow, const bool first) {
@@ -309,7 +311,7 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
             // exponents are set once, in the first pass, and the careful form stays cold afterwards
             const int kk = (k + (G::E * G::E) / 2) % (G::E * G::E);
             const int tz = kk / G::E, ty = kk % G::E;   // offset + M
-            const float2 *bRow = ((ty & 1) ? sBO : sBE) + (tz * G::NPE + l + (ty >> 1)) * G::PB2 + x0;
+            const float2 *bRow = ((ty & 1) ? sBO : sBE) + (tz * G::NPB + l + (ty >> 1)) * G::PB2 + x0;
             run_chunk(std::integral_constant<int, C::W0>{}, bRow, k == 0);
             if constexpr (C::W1 > 0) run_chunk(std::integral_constant<int, C::W1>{}, bRow + 4, false);
         }
@@ -402,15 +404,15 @@ inline const char *pair_name(const tnlm_params &p)
     }
 }
 
-template <int M, int RZ, int TX>
+template <int M, int RZ, int TX, int NCTA>
 cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, float *f_out, cudaStream_t st)
 {
     using G = PairGeom<M, RZ, TX>;
-    static_assert(G::BYTES <= 227 * 1024, "pair kernel tile does not fit in shared memory");
+    static_assert(NCTA * (G::BYTES + 1024) <= 228 * 1024, "NCTA tiles of the pair kernel do not fit in shared memory");
     static bool configured = false;   // per template instance; the attribute is idempotent
     cudaError_t e;
     if (!configured) {
-        e = cudaFuncSetAttribute(tnlm_pair_kernel<M, RZ, TX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
+        e = cudaFuncSetAttribute(tnlm_pair_kernel<M, RZ, TX, NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -419,7 +421,7 @@ cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, float 
     const int tiles_z = (dm.z_end + RZ - 1) / RZ - dm.z_begin / RZ;   // tiles aligned to multiples of RZ
     const long long blocks = (long long)tiles_x * tiles_y * tiles_z * dm.P;
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
-    tnlm_pair_kernel<M, RZ, TX><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
+    tnlm_pair_kernel<M, RZ, TX, NCTA><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
     return cudaGetLastError();
 }
 
@@ -429,21 +431,26 @@ inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float
 {
     if (ref != f) return cudaErrorNotSupported;
     switch (p.search_radius) {
-        case 1: return launch_pair_t<1, 8, 16>(dm, f, g, f_out, st);
+        case 1: {
+            static const int rz = tiled_env("TNLM_PAIR_RZ1", 43);
+            if (rz == 43) return launch_pair_t<1, 4, 16, 3>(dm, f, g, f_out, st);
+            return launch_pair_t<1, 8, 16, 2>(dm, f, g, f_out, st);
+        }
         case 2: {
-            static const int rz = tiled_env("TNLM_PAIR_RZ", 4);   // tuning knob for experiments
+            static const int rz = tiled_env("TNLM_PAIR_RZ", 43);   // tuning knob for experiments
             static const int tx = tiled_env("TNLM_PAIR_TX", 16);
-            if (tx == 24) return launch_pair_t<2, 4, 24>(dm, f, g, f_out, st);
-            if (rz == 6) return launch_pair_t<2, 6, 16>(dm, f, g, f_out, st);
-            if (rz == 4) return launch_pair_t<2, 4, 16>(dm, f, g, f_out, st);
-            return launch_pair_t<2, 8, 16>(dm, f, g, f_out, st);
+            if (tx == 24) return launch_pair_t<2, 4, 24, 2>(dm, f, g, f_out, st);
+            if (rz == 6) return launch_pair_t<2, 6, 16, 2>(dm, f, g, f_out, st);
+            if (rz == 4) return launch_pair_t<2, 4, 16, 2>(dm, f, g, f_out, st);
+            if (rz == 43) return launch_pair_t<2, 4, 16, 3>(dm, f, g, f_out, st);
+            return launch_pair_t<2, 8, 16, 2>(dm, f, g, f_out, st);
         }
         case 3: {
             static const int tx = tiled_env("TNLM_PAIR_TX3", 32);
-            if (tx == 16) return launch_pair_t<3, 4, 16>(dm, f, g, f_out, st);
-            return launch_pair_t<3, 6, 32>(dm, f, g, f_out, st);
+            if (tx == 16) return launch_pair_t<3, 4, 16, 2>(dm, f, g, f_out, st);
+            return launch_pair_t<3, 6, 32, 1>(dm, f, g, f_out, st);
         }
-        case 4: return launch_pair_t<4, 4, 32>(dm, f, g, f_out, st);
+        case 4: return launch_pair_t<4, 4, 32, 1>(dm, f, g, f_out, st);
         default: return cudaErrorNotSupported;
     }
 }
