@@ -8,6 +8,7 @@
 #include "tnlm_generic.cuh"
 #include "tnlm_tiled.cuh"
 #include "tnlm_pair.cuh"
+#include "tnlm_pair5.cuh"
 
 namespace {
 
@@ -61,8 +62,8 @@ int pick_variant(const tnlm_params *p, int variant)
 {
     if (variant == TNLM_VARIANT_GENERIC) return TNLM_VARIANT_GENERIC;
     if (variant == TNLM_VARIANT_TILED) return tiled_supported(*p) ? TNLM_VARIANT_TILED : -1;
-    if (variant == TNLM_VARIANT_PAIRED) return pair_supported(*p) ? TNLM_VARIANT_PAIRED : -1;
-    if (variant == TNLM_VARIANT_AUTO) return pair_supported(*p) ? TNLM_VARIANT_PAIRED : TNLM_VARIANT_GENERIC;
+    if (variant == TNLM_VARIANT_PAIRED) return (pair_supported(*p) || pair5_supported(*p)) ? TNLM_VARIANT_PAIRED : -1;
+    if (variant == TNLM_VARIANT_AUTO) return (pair_supported(*p) || pair5_supported(*p)) ? TNLM_VARIANT_PAIRED : TNLM_VARIANT_GENERIC;
     return -1;
 }
 
@@ -73,7 +74,7 @@ int launch_sweep(const tnlm_params *p, const float *f, const float *g, const flo
     if (z1 <= z0) return TNLM_OK;
     const Dims dm = make_dims(*p, z0, z1);
     if (variant == TNLM_VARIANT_PAIRED) {
-        cudaError_t e = launch_pair(*p, dm, f, g, ref, f_out, st);
+        cudaError_t e = p->patch_radius == 2 ? launch_pair5(*p, dm, f, g, ref, f_out, st) : launch_pair(*p, dm, f, g, ref, f_out, st);
         return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "paired sweep launch");
     }
     if (variant == TNLM_VARIANT_TILED) {
@@ -280,6 +281,7 @@ const char *tnlm_strerror(int code)
 const char *tnlm_kernel_name(const tnlm_params *p)
 {
     if (check_params(p) != TNLM_OK) return "invalid";
+    if (pair5_supported(*p)) return pair5_name(*p);
     return pair_supported(*p) ? pair_name(*p) : "jacobi_generic_kernel";
 }
 

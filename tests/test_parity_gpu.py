@@ -23,10 +23,13 @@ def T():
 
 
 def variants(T, p):
+    """Every kernel variant compiled for these parameters (include/tnlm.h: TNLM_VARIANT_*)."""
     out = [T.VARIANT_GENERIC]
-    if T.kernel_name(p) != "jacobi_generic_kernel":
-        out.append(T.VARIANT_TILED)
-        out.append(T.VARIANT_PAIRED)
+    if 1 <= p.search_radius <= 4:
+        if p.patch_radius == 1:
+            out.append(T.VARIANT_TILED)
+        if p.patch_radius in (1, 2):
+            out.append(T.VARIANT_PAIRED)
     return out
 
 
@@ -88,6 +91,9 @@ EDGE = [
     ((5, 2, 31, 129),   1, 2, 0.05,  0.5),    # flat slab, ragged x
     ((3, 17, 3, 4),     1, 1, 0.02,  0.5),    # tiny h: exponents in the thousands (reading P3)
     ((3, 4, 5, 6),      3, 1, 0.5,   0.5),    # largest compiled patch radius
+    ((2, 7, 33, 21),    2, 3, 0.15,  0.5),    # 5^3 patch, 7^3 window
+    ((2, 6, 29, 35),    2, 4, 0.15,  0.5),    # 5^3 patch, 9^3 window
+    ((3, 13, 57, 18),   2, 2, 0.12,  1.0),    # 5^3 patch over two y-tiles (28 output rows each)
 ]
 
 
@@ -125,6 +131,17 @@ def test_moving_edges_rebase_path(T, oracle, M, shape):
     for v in variants(T, p):
         got = T.tnlm_enhance(p, dev(g), 2, variant=v).cpu().numpy()
         assert_parity(got, want, dynamic_range(g), f"moving block M={M} variant {v}")
+
+
+@pytest.mark.parametrize("M,shape", [(1, (3, 9, 30, 20)), (2, (3, 10, 33, 22)), (3, (2, 9, 31, 18))])
+def test_moving_edges_rebase_path_patch5(T, oracle, M, shape):
+    g = moving_block_stack(shape, min(M, 2), 21 + M)
+    h, mu = 0.08, 0.5
+    p = T.TnlmParams.make(shape, 2, M, h, mu)
+    want = oracle.enhance(g, 2, M, np.float32(h), np.float32(mu), 2)
+    for v in variants(T, p):
+        got = T.tnlm_enhance(p, dev(g), 2, variant=v).cpu().numpy()
+        assert_parity(got, want, dynamic_range(g), f"moving block d=2 M={M} variant {v}")
 
 
 RAGGED = [(2, 7, 29, 15), (2, 5, 30, 16), (2, 4, 31, 17), (2, 13, 61, 47), (3, 6, 1, 50), (3, 1, 64, 2)]
