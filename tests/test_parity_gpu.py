@@ -296,3 +296,10 @@ def test_config4_shape_sampled(T, oracle):
     """Clinical-scale recipe (7^3 window, Z = 100 not a power of two) on a quarter in-plane grid."""
     cfg = CONFIGS["config4"].scaled(ny=256, nx=256, tumour_radius=8, si_amplitude=6)
     _sampled_step_parity(T, oracle, cfg, 3000, "config4 (256x256x100)")
+
+
+@pytest.mark.parametrize("d,M,n", [(2, 2, 1500), (1, 4, 1500), (2, 4, 400)])
+def test_config5_points_sampled(T, oracle, d, M, n):
+    """Points of the config-5 parameter sweep (5^3 patch, 9^3 window) at full in-plane size, 6 phases."""
+    cfg = CONFIGS["config5"].scaled(n_phase=6, nz=48, patch_radius=d, search_radius=M)
+    _sampled_step_parity(T, oracle, cfg, n, f"config5 d={d} M={M}")
