@@ -132,6 +132,29 @@ int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const fl
                                   float *f_out, int32_t z_begin, int32_t z_end, void *ws, size_t ws_bytes,
                                   void *cuda_stream, int variant);
 
+/*
+ * Image-quality metrics of the paper (evaluation, not on the TNLM-E hot path).
+ *
+ * tnlm_tv_diff: tv_out[p] = TV(a_p - b_p) for every phase p, TV(h) = int dx |grad h(x)| (the
+ *   seminorm of Eq. 10).  b == NULL means TV(a_p).  Discretisation (the paper gives none; M3): forward
+ *   differences at unit voxel spacing, a difference that would reach outside the volume is 0,
+ *   |grad h| = sqrt(hx^2 + hy^2 + hz^2) per voxel in fp32, plain sum over the voxels of the phase in fp64.
+ * tnlm_srr: srr_out[p] = [TV(f_fdk_p - f_star_p) - TV(f_enh_p - f_star_p)] / TV(f_fdk_p - f_star_p)  (Eq. 10).
+ *   ws: device scratch of at least 2 * n_phase * 8 bytes, 8-byte aligned.
+ * tnlm_cnr: out5 = { S, sigma, S_b, sigma_b, CNR } with CNR = 2 |S - S_b| / (sigma + sigma_b) for
+ *   the voxels of `phase` inside the half-open boxes roi / roi_bg = { z0, z1, y0, y1, x0, x1 } (HOST arrays of
+ *   6 int32, read before the call returns); sigma = population standard deviation.
+ * tv_out, srr_out (n_phase doubles) and out5 (5 doubles) are DEVICE pointers, 8-byte aligned.  The stack
+ * arguments follow the rules at the top of this file; patch_radius, search_radius, h, mu of `p` are ignored
+ * but must be valid.  Errors: TNLM_ERR_NULL_POINTER, TNLM_ERR_BAD_DIMS (phase or a box outside the volume,
+ * empty box), TNLM_ERR_WORKSPACE (misaligned pointer, ws too small), TNLM_ERR_CUDA.
+ */
+int tnlm_tv_diff(const tnlm_params *p, const float *a, const float *b, double *tv_out, void *cuda_stream);
+int tnlm_srr(const tnlm_params *p, const float *f_fdk, const float *f_enh, const float *f_star, double *srr_out,
+             void *ws, size_t ws_bytes, void *cuda_stream);
+int tnlm_cnr(const tnlm_params *p, const float *stack, int32_t phase, const int32_t *roi, const int32_t *roi_bg,
+             double *out5, void *cuda_stream);
+
 /* Message for a status code; for TNLM_ERR_CUDA includes the calling thread's last CUDA error text. */
 const char *tnlm_strerror(int code);
 

@@ -17,7 +17,8 @@ VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED = 0, 1, 2, 3
 EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_jacobi_step",
            "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
            "tnlm_enhance_host", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
-           "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count"]
+           "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
+           "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr"]
 
 
 class TnlmParams(C.Structure):
@@ -71,6 +72,9 @@ def lib():
         L.tnlm_strerror.argtypes = [C.c_int]; L.tnlm_strerror.restype = C.c_char_p
         L.tnlm_kernel_name.argtypes = [pp]; L.tnlm_kernel_name.restype = C.c_char_p
         L.tnlm_launches_per_sweep.argtypes = [pp]; L.tnlm_launches_per_sweep.restype = i32
+        L.tnlm_tv_diff.argtypes = [pp, vp, vp, vp, vp]
+        L.tnlm_srr.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp]
+        L.tnlm_cnr.argtypes = [pp, vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), vp, vp]
         L.tnlm_probe_fp32.argtypes = [i32, vp, vp]
         L.tnlm_probe_fp32_ffma_count.argtypes = [i32]; L.tnlm_probe_fp32_ffma_count.restype = C.c_double
         _LIB = L
@@ -209,3 +213,34 @@ def probe_fp32(n_iter: int, sink, stream=None) -> float:
     """Enqueue the FFMA probe; returns the number of FFMA lane-operations it executes."""
     _check(lib().tnlm_probe_fp32(int(n_iter), sink.data_ptr(), _stream(stream)), "tnlm_probe_fp32")
     return float(lib().tnlm_probe_fp32_ffma_count(int(n_iter)))
+
+
+def tnlm_tv_diff(p: TnlmParams, a, b=None, stream=None):
+    """TV(a_p - b_p) per phase (Eq. 10's seminorm; see include/tnlm.h) -> float64 CUDA tensor [n_phase]."""
+    import torch
+    out = torch.empty(p.n_phase, dtype=torch.float64, device=a.device)
+    _check(lib().tnlm_tv_diff(C.byref(p), _dev_ptr(a, p, "a"), _dev_ptr(b, p, "b", optional=True), out.data_ptr(),
+                              _stream(stream)), "tnlm_tv_diff")
+    return out
+
+
+def tnlm_srr(p: TnlmParams, f_fdk, f_enh, f_star, stream=None):
+    """Streak-reduction ratio of Eq. 10 per phase -> float64 CUDA tensor [n_phase]."""
+    import torch
+    out = torch.empty(p.n_phase, dtype=torch.float64, device=f_fdk.device)
+    ws = torch.empty(2 * p.n_phase, dtype=torch.float64, device=f_fdk.device)
+    _check(lib().tnlm_srr(C.byref(p), _dev_ptr(f_fdk, p, "f_fdk"), _dev_ptr(f_enh, p, "f_enh"),
+                          _dev_ptr(f_star, p, "f_star"), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
+                          _stream(stream)), "tnlm_srr")
+    return out
+
+
+def tnlm_cnr(p: TnlmParams, stack, phase, roi, roi_bg, stream=None):
+    """[S, sigma, S_b, sigma_b, CNR] of two half-open boxes (z0, z1, y0, y1, x0, x1) of `phase`."""
+    import torch
+    out = torch.empty(5, dtype=torch.float64, device=stack.device)
+    r0 = (C.c_int32 * 6)(*[int(v) for v in roi])
+    r1 = (C.c_int32 * 6)(*[int(v) for v in roi_bg])
+    _check(lib().tnlm_cnr(C.byref(p), _dev_ptr(stack, p, "stack"), int(phase), r0, r1, out.data_ptr(),
+                          _stream(stream)), "tnlm_cnr")
+    return out

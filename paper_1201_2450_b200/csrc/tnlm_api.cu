@@ -9,6 +9,7 @@
 #include "tnlm_tiled.cuh"
 #include "tnlm_pair.cuh"
 #include "tnlm_pair5.cuh"
+#include "tnlm_metrics.cuh"
 
 namespace {
 
@@ -261,6 +262,76 @@ int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_
     if (e != cudaSuccess) return cuda_fail(e, "D2H f_out");
     e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "enhance_host sync");
+}
+
+int tnlm_tv_diff(const tnlm_params *p, const float *a, const float *b, double *tv_out, void *cuda_stream)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!a || !tv_out) return TNLM_ERR_NULL_POINTER;
+    if (misaligned(a) || misaligned(b) || ((uintptr_t)tv_out & 7u)) return TNLM_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMemsetAsync(tv_out, 0, sizeof(double) * p->n_phase, st);
+    if (e != cudaSuccess) return cuda_fail(e, "tv memset");
+    const size_t groups = (size_t)p->nz * p->ny * ((p->nx + 3) / 4);
+    size_t blocks = (groups + kMetricThreads - 1) / kMetricThreads;
+    const size_t cap = (size_t)sm_count() * 16 / (size_t)p->n_phase + 1;   // ~16 CTAs (two full waves of 8) per SM over all phases
+    if (blocks > cap) blocks = cap;
+    tv_diff_kernel<<<dim3((unsigned)blocks, (unsigned)p->n_phase), kMetricThreads, 0, st>>>(a, b, tv_out, p->nz, p->ny, p->nx);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "tv launch");
+}
+
+int tnlm_srr(const tnlm_params *p, const float *f_fdk, const float *f_enh, const float *f_star, double *srr_out,
+             void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!f_fdk || !f_enh || !f_star || !srr_out) return TNLM_ERR_NULL_POINTER;
+    if (!ws || ((uintptr_t)ws & 7u) || ((uintptr_t)srr_out & 7u) || ws_bytes < 2 * sizeof(double) * (size_t)p->n_phase)
+        return TNLM_ERR_WORKSPACE;
+    double *t = (double *)ws;
+    rc = tnlm_tv_diff(p, f_fdk, f_star, t, cuda_stream);
+    if (rc) return rc;
+    rc = tnlm_tv_diff(p, f_enh, f_star, t + p->n_phase, cuda_stream);
+    if (rc) return rc;
+    srr_finish_kernel<<<(p->n_phase + 63) / 64, 64, 0, (cudaStream_t)cuda_stream>>>(t, srr_out, p->n_phase);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "srr launch");
+}
+
+int tnlm_cnr(const tnlm_params *p, const float *stack, int32_t phase, const int32_t *roi, const int32_t *roi_bg,
+             double *out5, void *cuda_stream)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!stack || !roi || !roi_bg || !out5) return TNLM_ERR_NULL_POINTER;
+    if (misaligned(stack) || ((uintptr_t)out5 & 7u)) return TNLM_ERR_WORKSPACE;
+    if (phase < 0 || phase >= p->n_phase) return TNLM_ERR_BAD_DIMS;
+    Box bx[2];
+    const int32_t *src[2] = {roi, roi_bg};
+    double n[2];
+    for (int r = 0; r < 2; ++r) {
+        const int32_t *q = src[r];
+        if (q[0] < 0 || q[1] > p->nz || q[0] >= q[1] || q[2] < 0 || q[3] > p->ny || q[2] >= q[3] || q[4] < 0 ||
+            q[5] > p->nx || q[4] >= q[5])
+            return TNLM_ERR_BAD_DIMS;
+        bx[r] = Box{q[0], q[1], q[2], q[3], q[4], q[5]};
+        n[r] = (double)(q[1] - q[0]) * (q[3] - q[2]) * (q[5] - q[4]);
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMemsetAsync(out5, 0, 5 * sizeof(double), st);
+    if (e != cudaSuccess) return cuda_fail(e, "cnr memset");
+    const double nmax = n[0] > n[1] ? n[0] : n[1];
+    size_t blocks = (size_t)((nmax + kMetricThreads - 1) / kMetricThreads);
+    const size_t cap = (size_t)sm_count() * 4;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    const float *vol = stack + (size_t)phase * p->nz * p->ny * p->nx;
+    roi_sums_kernel<<<dim3((unsigned)blocks, 2), kMetricThreads, 0, st>>>(vol, p->ny, p->nx, bx[0], bx[1], 0.f, out5);
+    cnr_finish_kernel<<<1, 32, 0, st>>>(out5, n[0], n[1], 0.f, out5);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "cnr launch");
 }
 
 const char *tnlm_strerror(int code)
