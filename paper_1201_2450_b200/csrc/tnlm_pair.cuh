@@ -195,7 +195,7 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
 //   dstE pair r/2 (half r&1); dstO (optional) pair (r-1)/2 (half (r-1)&1) for r >= 1
 // The (r, c) of a thread's k-th element is the same in every plane, so its global offset inside a
 // plane and its shared-memory offsets are tabulated once; the plane loop is then LDG + STS only,
-// four planes (4K loads) in flight per thread.
+// four or five planes in flight per thread.
 template <int PITCH2, int ROWS, int COLS, int PLANES, int NP, int NPO, bool NEGATE, int NT>
 __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__restrict__ dstO,
                                             const float *__restrict__ src, const int zo, const int yo, const int xo,
@@ -204,7 +204,7 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
     constexpr int K = (ROWS * COLS + NT - 1) / NT;
     constexpr bool ODD = NPO > 0;
     constexpr int PLANE_F = (NP + NPO) * PITCH2 * 2;   // floats per shared-memory plane (even pairs, then odd pairs)
-    constexpr int PF = 4;                      // planes in flight
+    constexpr int PF = (PLANES % 5 == 0 && K <= 8) ? 5 : 4;   // planes in flight
     int goff[K], eoff[K], ooff[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
