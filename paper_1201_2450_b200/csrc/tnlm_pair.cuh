@@ -204,7 +204,7 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
     constexpr int K = (ROWS * COLS + NT - 1) / NT;
     constexpr bool ODD = NPO > 0;
     constexpr int PLANE_F = (NP + NPO) * PITCH2 * 2;   // floats per shared-memory plane (even pairs, then odd pairs)
-    constexpr int PF = (PLANES % 5 == 0 && K <= 8) ? 5 : 4;   // planes in flight
+    constexpr int PF = (PLANES % 7 == 0 && K <= 4) ? 7 : (PLANES % 5 == 0 && K <= 8) ? 5 : 4;   // planes in flight
     int goff[K], eoff[K], ooff[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
