@@ -430,28 +430,11 @@ inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float
                                float *f_out, cudaStream_t st)
 {
     if (ref != f) return cudaErrorNotSupported;
+    // <M, RZ, TX, CTAs per SM>: the shapes that measured best on the thorax phantoms
     switch (p.search_radius) {
-        case 1: {
-            static const int rz = tiled_env("TNLM_PAIR_RZ1", 43);
-            if (rz == 43) return launch_pair_t<1, 4, 16, 3>(dm, f, g, f_out, st);
-            return launch_pair_t<1, 8, 16, 2>(dm, f, g, f_out, st);
-        }
-        case 2: {
-            static const int rz = tiled_env("TNLM_PAIR_RZ", 43);   // tuning knob for experiments
-            static const int tx = tiled_env("TNLM_PAIR_TX", 16);
-            if (tx == 24) return launch_pair_t<2, 4, 24, 2>(dm, f, g, f_out, st);
-            if (rz == 6) return launch_pair_t<2, 6, 16, 2>(dm, f, g, f_out, st);
-            if (rz == 5) return launch_pair_t<2, 5, 16, 2>(dm, f, g, f_out, st);
-            if (rz == 4) return launch_pair_t<2, 4, 16, 2>(dm, f, g, f_out, st);
-            if (rz == 43) return launch_pair_t<2, 4, 16, 3>(dm, f, g, f_out, st);
-            return launch_pair_t<2, 8, 16, 2>(dm, f, g, f_out, st);
-        }
-        case 3: {
-            static const int tx = tiled_env("TNLM_PAIR_TX3", 32);
-            if (tx == 16) return launch_pair_t<3, 4, 16, 2>(dm, f, g, f_out, st);
-            if (tx == 324) return launch_pair_t<3, 4, 32, 1>(dm, f, g, f_out, st);
-            return launch_pair_t<3, 6, 32, 1>(dm, f, g, f_out, st);
-        }
+        case 1: return launch_pair_t<1, 4, 16, 3>(dm, f, g, f_out, st);
+        case 2: return launch_pair_t<2, 4, 16, 3>(dm, f, g, f_out, st);
+        case 3: return launch_pair_t<3, 6, 32, 1>(dm, f, g, f_out, st);
         case 4: return launch_pair_t<4, 4, 32, 1>(dm, f, g, f_out, st);
         default: return cudaErrorNotSupported;
     }

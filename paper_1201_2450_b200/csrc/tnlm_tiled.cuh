@@ -385,22 +385,10 @@ cudaError_t launch_tiled_t(const Dims &dm, const float *f, const float *g, float
     return cudaGetLastError();
 }
 
-inline int tiled_env(const char *name, int dflt)
-{
-    const char *e = getenv(name);   // tuning knobs for experiments; defaults are the shipped configuration
-    return e ? atoi(e) : dflt;
-}
-
 template <int M>
 cudaError_t launch_tiled_m(const Dims &dm, const float *f, const float *g, float *f_out, cudaStream_t st)
 {
-    static const int xr = tiled_env("TNLM_TILED_XR", kTiledXR), rz = tiled_env("TNLM_TILED_RZ", kTiledRZ);
-    if (xr == 4) {
-        if (rz == 6) return launch_tiled_t<M, 4, 6>(dm, f, g, f_out, st);
-        return launch_tiled_t<M, 4, 8>(dm, f, g, f_out, st);
-    }
-    if (rz == 6) return launch_tiled_t<M, 2, 6>(dm, f, g, f_out, st);
-    return launch_tiled_t<M, 2, 8>(dm, f, g, f_out, st);
+    return launch_tiled_t<M, kTiledXR, kTiledRZ>(dm, f, g, f_out, st);
 }
 
 // ref must be f (TNLM-E); the caller falls back to the generic kernel otherwise.
