@@ -53,7 +53,11 @@ typedef enum {
     TNLM_ERR_CUDA = -7          /* a CUDA call failed; tnlm_strerror(TNLM_ERR_CUDA) has the text   */
 } tnlm_status;
 
-/* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M). */
+/* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M):
+ *   GENERIC  any d <= 3, M <= 6, any ref: one thread per voxel, loops as the definition
+ *   TILED    d = 1, 1 <= M <= 4, ref == f: scalar FP32 tiles (first optimised kernel, kept for cross-checks)
+ *   PAIRED   d = 1 or 2, 1 <= M <= 4, ref == f: row-pair packed FP32 (FADD2 / FFMA2) -- what AUTO selects there
+ * With AUTO a separate ref (ref != f) takes GENERIC. */
 enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2, TNLM_VARIANT_PAIRED = 3 };
 
 /*
