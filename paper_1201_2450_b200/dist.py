@@ -116,3 +116,24 @@ def exchange_halos(info: RankInfo, stack, halo: int):
     for buf, lo, hi in keep:
         stack[:, lo:hi].copy_(buf)
     return stack
+
+
+def enhance_z_slabs(info: RankInfo, g, n_iter: int, halo: int, sweep_slab):
+    """TNLM-E on ONE stack sharded by z-slab over the ranks.
+
+    Every rank holds full-size arrays `[P][Z][Y][X]` but owns only its slab `[a, b)` of planes (`z_slab`): per
+    Gauss-Jacobi sweep it refreshes the `halo = M + d` planes next to its slab from its z-neighbours
+    (`exchange_halos`, point-to-point, no reduction) and then computes its slab of Eq. 8 from the old iterate.
+    `sweep_slab(f, g, a, b, out)` must write `out[:, a:b]` (on the GPUs: `tnlm_jacobi_step_slab`; the CPU tests
+    pass the oracle).  Returns `(f, (a, b))`: the rank's copy after `n_iter` sweeps (valid in `[a, b)`) and its slab.
+    Slab results equal the single-device sweep bit for bit (z-tiles are aligned to absolute plane indices).
+    """
+    Z = g.shape[1]
+    a, b = z_slab(Z, info.rank, info.world)
+    f = g.clone()
+    out = g.clone()
+    for _ in range(int(n_iter)):
+        exchange_halos(info, f, halo)
+        sweep_slab(f, g, a, b, out)
+        f, out = out, f
+    return f, (a, b)

@@ -67,6 +67,42 @@ def _worker(rank, world, port, shape, d, M, h, mu, n_sweeps, out_dir):
     D.finalize(info)
 
 
+def _worker_enhance(rank, world, port, shape, d, M, h, mu, n_sweeps, out_dir):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    from oracle import tnlm_oracle as O
+    from tnlm_inputs import random_stack
+
+    info = D.init("gloo")
+    P, Z, Y, X = shape
+    g = torch.from_numpy(random_stack(shape, 7))
+    plane = Y * X
+
+    def sweep_slab(f, gg, a, b, out):
+        own = (np.arange(P)[:, None] * Z * plane + np.arange(a * plane, b * plane)[None, :]).reshape(-1).astype(np.int64)
+        new = O.jacobi_step_at(f.numpy(), gg.numpy(), d, M, np.float32(h), np.float32(mu), own)
+        out.view(-1)[torch.from_numpy(own)] = torch.from_numpy(new)
+
+    f, (a, b) = D.enhance_z_slabs(info, g, n_sweeps, M + d, sweep_slab)
+    np.save(os.path.join(out_dir, f"enh{rank}.npy"), f[:, a:b].numpy())
+    D.barrier(info)
+    D.finalize(info)
+
+
+def test_enhance_z_slabs_two_ranks_equals_single_process(tmp_path, oracle):
+    import torch.multiprocessing as mp
+    shape, d, M, h, mu, n_sweeps, world = (3, 9, 6, 7), 1, 2, 0.3, 0.7, 3, 2
+    mp.spawn(_worker_enhance, args=(world, _free_port(), shape, d, M, h, mu, n_sweeps, str(tmp_path)), nprocs=world,
+             join=True)
+    from tnlm_inputs import random_stack
+    g = random_stack(shape, 7)
+    want = oracle.enhance(g, d, M, np.float32(h), np.float32(mu), n_sweeps)
+    got = np.concatenate([np.load(tmp_path / f"enh{r}.npy") for r in range(world)], axis=1)
+    assert np.array_equal(got, want)
+
+
 def test_z_slabs_tile_the_volume():
     from paper_1201_2450_b200 import dist as D
     for n in (1, 5, 16, 100, 128):

@@ -303,3 +303,30 @@ def test_config5_points_sampled(T, oracle, d, M, n):
     """Points of the config-5 parameter sweep (5^3 patch, 9^3 window) at full in-plane size, 6 phases."""
     cfg = CONFIGS["config5"].scaled(n_phase=6, nz=48, patch_radius=d, search_radius=M)
     _sampled_step_parity(T, oracle, cfg, n, f"config5 d={d} M={M}")
+
+
+def test_enhance_z_slabs_driver_matches_tnlm_enhance_bitwise(T):
+    """The multi-GPU z-slab driver (dist.enhance_z_slabs) with the CUDA slab sweep; one process here, so the
+    halo exchange is a no-op and the slab is the whole stack: it must reproduce tnlm_enhance bit for bit.  A split
+    into two slabs on the same device (what two ranks would compute) must as well."""
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    shape = (4, 19, 33, 40)
+    g = dev(random_stack(shape, 41))
+    p = T.TnlmParams.make(shape, 1, 2, 0.2, 0.5)
+    want = T.tnlm_enhance(p, g, 3)
+    info = D.RankInfo(0, 0, 1)
+
+    def sweep(f, gg, a, b, out):
+        T.tnlm_jacobi_step_slab(p, f, gg, a, b, f_out=out)
+
+    got, (a, b) = D.enhance_z_slabs(info, g, 3, 3, sweep)
+    assert (a, b) == (0, shape[1]) and torch.equal(got, want)
+
+    def sweep_two(f, gg, a, b, out):          # the two slabs two ranks would own
+        for r in range(2):
+            za, zb = D.z_slab(shape[1], r, 2)
+            T.tnlm_jacobi_step_slab(p, f, gg, za, zb, f_out=out)
+
+    got2, _ = D.enhance_z_slabs(info, g, 3, 3, sweep_two)
+    assert torch.equal(got2, want)
