@@ -32,7 +32,8 @@
 // normaliser stays below 2^100 (no candidate ~2^100 times better than the reference) it is added as
 // it is; otherwise (first use, b = +inf; later only at moving high-contrast edges) nothing is added,
 // the row pair is flagged, and the warp re-does that pass in a careful form that re-bases flagged
-// pairs on min(b, c2*Dmin of the pass) and re-evaluates their terms.  The result equals the shifted
+// pairs on min(b, c2*Dmin of the pass - 90) and re-evaluates their terms (the 90 binades of headroom make a
+// second re-base of the same output rare even on noise-dominated stacks).  The result equals the shifted
 // softmax up to rounding.
 #pragma once
 #include <cstdlib>
@@ -76,6 +77,9 @@ template <int M, int RZ, int TX> struct PairGeom {
 
 struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
 
+// A re-base puts the best candidate seen so far at 2^-90, not at 1: later candidates may be up to 2^190 times better
+// before the guard trips again, while terms down to 2^-36 of the best stay normal (125 * 2^-36 = 2e-9 of the sum).
+constexpr float kPairHead = 90.f;
 constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100: partial sums up to here are added as they are; Z < 2^107 (safe for __fdividef)
 
 template <int NV>
@@ -161,9 +165,12 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                         float2 dmin = D[0];
 #pragma unroll
                         for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
-                        const float2 nb = make_float2(fminf(c2 * dmin.x, ac.b[i].x), fminf(c2 * dmin.y, ac.b[i].y));
-                        const float2 sc = make_float2(ex2(nb.x - ac.b[i].x), ex2(nb.y - ac.b[i].y));   // 1 if unchanged, 0 on first use
-                        float2 zz = mul2(ac.z[i], sc), nn = mul2(ac.n[i], sc);
+                        // only the row whose partial sum left the band is re-based (the other keeps its reference: sc = 1)
+                        const float2 nb = make_float2(zp.x <= kPairGuard ? ac.b[i].x : fminf(c2 * dmin.x - kPairHead, ac.b[i].x),
+                                                      zp.y <= kPairGuard ? ac.b[i].y : fminf(c2 * dmin.y - kPairHead, ac.b[i].y));
+                        // scale by 2^(nb - b) in two halves: the factor itself may be below 2^-126 when the product is not
+                        const float2 sc = make_float2(ex2(0.5f * (nb.x - ac.b[i].x)), ex2(0.5f * (nb.y - ac.b[i].y)));   // 1 if unchanged, 0 on first use
+                        float2 zz = mul2(mul2(ac.z[i], sc), sc), nn = mul2(mul2(ac.n[i], sc), sc);
 #pragma unroll
                         for (int q = 0; q < W; ++q) {
                             const float2 ar = fma2(D[q], nc2, nb);

@@ -98,9 +98,12 @@ __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, 
                         float2 dmin = D[0];
 #pragma unroll
                         for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
-                        const float2 nb = make_float2(fminf(c2 * dmin.x, ac.b[i].x), fminf(c2 * dmin.y, ac.b[i].y));
-                        const float2 sc = make_float2(ex2(nb.x - ac.b[i].x), ex2(nb.y - ac.b[i].y));   // 1 if unchanged, 0 on first use
-                        float2 zz = mul2(ac.z[i], sc), nn = mul2(ac.n[i], sc);
+                        // only the row whose partial sum left the band is re-based (the other keeps its reference: sc = 1)
+                        const float2 nb = make_float2(zp.x <= kPairGuard ? ac.b[i].x : fminf(c2 * dmin.x - kPairHead, ac.b[i].x),
+                                                      zp.y <= kPairGuard ? ac.b[i].y : fminf(c2 * dmin.y - kPairHead, ac.b[i].y));
+                        // scale by 2^(nb - b) in two halves: the factor itself may be below 2^-126 when the product is not
+                        const float2 sc = make_float2(ex2(0.5f * (nb.x - ac.b[i].x)), ex2(0.5f * (nb.y - ac.b[i].y)));   // 1 if unchanged, 0 on first use
+                        float2 zz = mul2(mul2(ac.z[i], sc), sc), nn = mul2(mul2(ac.n[i], sc), sc);
 #pragma unroll
                         for (int q = 0; q < W; ++q) {
                             const float2 ar = fma2(D[q], nc2, nb);
