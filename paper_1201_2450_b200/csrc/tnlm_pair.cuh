@@ -77,10 +77,13 @@ template <int M, int RZ, int TX> struct PairGeom {
 
 struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
 
+// Guard band and headroom of the reference exponents.  Partial sums up to 2^100 (relative to the reference) are added
+// as they are: Z stays below 2^107 (inside __fdividef's range) and N below 2^107 * max|f|, finite for |f| < 2^20
+// (a 2^80 band would cover |f| < 2^40 but re-bases noise-dominated stacks 15 % more often).
 // A re-base puts the best candidate seen so far at 2^-90, not at 1: later candidates may be up to 2^190 times better
 // before the guard trips again, while terms down to 2^-36 of the best stay normal (125 * 2^-36 = 2e-9 of the sum).
 constexpr float kPairHead = 90.f;
-constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100: partial sums up to here are added as they are; Z < 2^107 (safe for __fdividef)
+constexpr float kPairGuard = 1.2676506002282294e30f;   // 2^100
 
 template <int NV>
 __device__ __forceinline__ void load_pairs(const float2 *__restrict__ p, float2 (&dst)[2 * NV])
