@@ -330,3 +330,20 @@ def test_enhance_z_slabs_driver_matches_tnlm_enhance_bitwise(T):
 
     got2, _ = D.enhance_z_slabs(info, g, 3, 3, sweep_two)
     assert torch.equal(got2, want)
+
+
+@pytest.mark.parametrize("scale", [1e-3, 4096.0])
+def test_scale_covariance(T, scale):
+    """Eq. 3 / Eq. 8 are covariant under g -> s g, h -> s h (the exponent is unchanged, the update is linear):
+    intensities in other units (HU-like thousands, or tiny) must give the scaled result; powers-of-two-free
+    scales exercise the exponent ranges of the accumulators."""
+    import torch
+    cfg = CONFIGS["config2"].scaled(nz=12, ny=40, nx=48, tumour_radius=3, si_amplitude=2)
+    g = make_stack(cfg)
+    for d, M in [(1, 2), (2, 1)]:
+        p1 = T.TnlmParams.make(cfg.shape, d, M, cfg.h, cfg.mu)
+        ps = T.TnlmParams.make(cfg.shape, d, M, cfg.h * scale, cfg.mu)
+        base = T.tnlm_enhance(p1, dev(g), 2).cpu().numpy().astype(np.float64)
+        got = T.tnlm_enhance(ps, dev((g.astype(np.float64) * scale).astype(np.float32)), 2).cpu().numpy().astype(np.float64)
+        assert np.isfinite(got).all()
+        assert_parity(got / scale, base, dynamic_range(g), f"scale {scale} d={d} M={M}")
