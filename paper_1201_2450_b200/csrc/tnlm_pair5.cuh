@@ -39,7 +39,7 @@ template <int M, int RZ, int TX> struct Pair5Geom {
 // CAREFUL as in pair_pass (tnlm_pair.cuh).
 template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE>
 __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
-                                               const float c2, AccPair (&acc)[RZ], const unsigned mask)
+                                               const float c2, AccPair (&acc)[RZ], const unsigned mask, const bool first = false)
 {
     constexpr int NVB = (W + 6) / 2;   // 6 + W - 1 positions
     const float2 nc2 = make_float2(-c2, -c2);
@@ -81,13 +81,18 @@ __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, 
                     D[q] = add2(make_float2(u0, d1), make_float2(common, common));
                 }
                 if (!CAREFUL || ((mask >> (2 * (p - 4) + i)) & 1u)) {
-                    float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
+                    // `first` (careful form only, warp-uniform): the accumulators are empty and the reference is
+                    // +inf, so the optimistic sum is skipped and the pair goes straight to the re-base
+                    float2 zp = make_float2(INFINITY, INFINITY), np = make_float2(0.f, 0.f);
+                    if (!CAREFUL || !first) {
+                        zp = make_float2(0.f, 0.f);
 #pragma unroll
-                    for (int q = 0; q < W; ++q) {
-                        const float2 arg = fma2(D[q], nc2, ac.b[i]);                      // a3
-                        const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
-                        zp = add2(zp, u);                                                 // a4
-                        np = fma2(u, cand2[i + q], np);
+                        for (int q = 0; q < W; ++q) {
+                            const float2 arg = fma2(D[q], nc2, ac.b[i]);                  // a3
+                            const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
+                            zp = add2(zp, u);                                             // a4
+                            np = fma2(u, cand2[i + q], np);
+                        }
                     }
                     if (fmaxf(zp.x, zp.y) <= kPairGuard) {
                         ac.z[i] = add2(ac.z[i], zp);
@@ -191,7 +196,7 @@ tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, floa
             constexpr int W = decltype(wtag)::value;
             unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
             if (!first) fail = pair5_pass<RZ, W, false, AP, BP>(aRow, bRow, dm.c2, acc, 0u);
-            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail, first);
         };
 #pragma unroll 1
         for (int k = 0; k < G::E * G::E; ++k) {
