@@ -38,7 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libtnlm.so")
     os.replace(tmp, LIB)
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as fh:
-        fh.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+        fh.write((" ".join(cmd) + "\n" + res.stdout + res.stderr).replace(tmp, LIB).replace(HERE + os.sep, ""))
     return LIB
 
 
