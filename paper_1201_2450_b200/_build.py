@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libtnlm.so")
     os.replace(tmp, LIB)
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as fh:
-        fh.write((" ".join(cmd) + "\n" + res.stdout + res.stderr).replace(tmp, LIB).replace(HERE + os.sep, ""))
+        log = (" ".join(cmd) + "\n" + res.stdout + res.stderr).replace(tmp, LIB).replace(HERE + os.sep, "")
+        fh.write("".join(ln for ln in log.splitlines(True) if "Compile time" not in ln))   # registers and spills, no timings
     return LIB
 
 
