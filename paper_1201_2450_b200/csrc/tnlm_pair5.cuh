@@ -299,7 +299,7 @@ inline cudaError_t launch_pair5(const tnlm_params &p, const Dims &dm, const floa
 {
     if (ref != f) return cudaErrorNotSupported;
     switch (p.search_radius) {
-        case 1: return launch_pair5_t<1, 4, 16, 2>(dm, f, g, f_out, st);
+        case 1: return launch_pair5_t<1, 6, 16, 2>(dm, f, g, f_out, st);
         case 2: return launch_pair5_t<2, 4, 16, 2>(dm, f, g, f_out, st);
         case 3: return launch_pair5_t<3, 4, 32, 1>(dm, f, g, f_out, st);
         case 4: return launch_pair5_t<4, 2, 32, 1>(dm, f, g, f_out, st);
