@@ -347,3 +347,25 @@ def test_scale_covariance(T, scale):
         got = T.tnlm_enhance(ps, dev((g.astype(np.float64) * scale).astype(np.float32)), 2).cpu().numpy().astype(np.float64)
         assert np.isfinite(got).all()
         assert_parity(got / scale, base, dynamic_range(g), f"scale {scale} d={d} M={M}")
+
+
+def test_fuzz_packed_kernels_against_generic(T):
+    """Seeded random shapes and parameters: the packed kernels (d = 1, 2; M = 1..4) against the generic kernel (which the
+    tests above tie to the oracle), one sweep each, including slabs that start and end off the z-tile grid."""
+    import torch
+    rng = np.random.default_rng(2024)
+    for case in range(28):
+        d = int(rng.integers(1, 3)); M = int(rng.integers(1, 5))
+        shape = (int(rng.integers(2, 5)), int(rng.integers(1, 14)), int(rng.integers(1, 70)), int(rng.integers(1, 50)))
+        h = float(rng.choice([0.03, 0.1, 0.4, 5.0])); mu = float(rng.choice([0.2, 1.0, 3.0]))
+        f, g = dev(random_stack(shape, 100 + case)), dev(random_stack(shape, 200 + case))
+        p = T.TnlmParams.make(shape, d, M, h, mu)
+        want = T.tnlm_jacobi_step(p, f, g, variant=T.VARIANT_GENERIC)
+        got = T.tnlm_jacobi_step(p, f, g, variant=T.VARIANT_PAIRED)
+        err = (got - want).abs().max().item()
+        assert err <= 1e-4, f"case {case}: shape {shape} d={d} M={M} h={h}: max|d|={err:.3e}"
+        za = int(rng.integers(0, shape[1])); zb = int(rng.integers(za, shape[1] + 1))
+        out = torch.full_like(f, -3.0)
+        T.tnlm_jacobi_step_slab(p, f, g, za, zb, f_out=out, variant=T.VARIANT_PAIRED)
+        assert torch.equal(out[:, za:zb], got[:, za:zb]), f"case {case}: slab [{za},{zb}) differs from the full sweep"
+        assert (out[:, :za] == -3.0).all() and (out[:, zb:] == -3.0).all(), f"case {case}: slab wrote outside [{za},{zb})"
