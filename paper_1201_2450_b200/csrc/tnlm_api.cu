@@ -236,6 +236,82 @@ int tnlm_enhance(const tnlm_params *p, const float *g, const float *f_init, floa
     return tnlm_enhance_variant(p, g, f_init, f_out, n_iter, ws, ws_bytes, cuda_stream, TNLM_VARIANT_AUTO);
 }
 
+// Pipelined form of tnlm_enhance_host (f_init == g, n_iter >= 1, volumes deep enough for four z-slabs): the stack
+// goes to the device slab by slab on an internal copy stream while the first sweep already runs on the slabs whose
+// planes (and M+d planes of halo) have arrived, and the last sweep hands its slabs back the same way.  Slab sweeps
+// are bit-identical to whole-volume sweeps (z-tiles are aligned to absolute plane indices), so the result equals
+// tnlm_enhance's bit for bit.
+static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, float *f_out_host, int32_t n_iter,
+                                  float *g_dev, float *fo_dev, void *ws, size_t ws_bytes, cudaStream_t st, int variant)
+{
+    constexpr int NS = 4;
+    const int halo = p->search_radius + p->patch_radius;
+    const size_t plane = (size_t)p->ny * p->nx, pitch = plane * p->nz * sizeof(float), sb = stack_bytes(p);
+    int zb[NS + 1];
+    for (int s = 0; s <= NS; ++s) zb[s] = (int)((long long)p->nz * s / NS) / 8 * 8;   // slab bounds on multiples of 8
+    zb[NS] = p->nz;
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev_in[NS] = {}, ev_out[NS] = {}, ev_start = nullptr;
+    cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return cuda_fail(e, "copy stream");
+    int rc = TNLM_OK;
+    auto fail = [&](cudaError_t err, const char *what) { rc = cuda_fail(err, what); };
+    auto ck = [&](cudaError_t err, const char *what) { if (err != cudaSuccess && rc == TNLM_OK) fail(err, what); return err == cudaSuccess; };
+    ck(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming), "event");
+    for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
+        ck(cudaEventCreateWithFlags(&ev_in[s], cudaEventDisableTiming), "event");
+        ck(cudaEventCreateWithFlags(&ev_out[s], cudaEventDisableTiming), "event");
+    }
+    if (rc == TNLM_OK) {
+        // the copy stream starts after whatever the caller queued on its stream before this call
+        ck(cudaEventRecord(ev_start, st), "event record");
+        ck(cudaStreamWaitEvent(cs, ev_start, 0), "stream wait");
+        for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
+            const size_t off = (size_t)zb[s] * plane;
+            ck(cudaMemcpy2DAsync(g_dev + off, pitch, g_host + off, pitch, (size_t)(zb[s + 1] - zb[s]) * plane * sizeof(float),
+                                 (size_t)p->n_phase, cudaMemcpyHostToDevice, cs), "H2D slab");
+            ck(cudaEventRecord(ev_in[s], cs), "event record");
+        }
+    }
+    float *buf_ws = (float *)ws;
+    char *kws = (char *)ws + align_up(sb, 256);
+    const size_t kws_bytes = ws_bytes - align_up(sb, 256);
+    const float *cur = g_dev;
+    float *dst = (n_iter % 2 == 1) ? fo_dev : buf_ws;
+    for (int k = 0; k < n_iter && rc == TNLM_OK; ++k) {
+        const bool first = k == 0, last = k == n_iter - 1;
+        if (!first && !last) {
+            rc = launch_sweep(p, cur, g_dev, cur, dst, 0, p->nz, kws, kws_bytes, st, variant);
+        } else {
+            for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
+                // slab s of the first sweep reads up to `halo` planes of slab s+1
+                if (first) ck(cudaStreamWaitEvent(st, ev_in[s + 1 < NS ? s + 1 : NS - 1], 0), "stream wait");
+                if (rc == TNLM_OK) rc = launch_sweep(p, cur, g_dev, cur, dst, zb[s], zb[s + 1], kws, kws_bytes, st, variant);
+                if (last && rc == TNLM_OK) {
+                    const size_t off = (size_t)zb[s] * plane;
+                    ck(cudaEventRecord(ev_out[s], st), "event record");
+                    ck(cudaStreamWaitEvent(cs, ev_out[s], 0), "stream wait");
+                    ck(cudaMemcpy2DAsync(f_out_host + off, pitch, dst + off, pitch,
+                                         (size_t)(zb[s + 1] - zb[s]) * plane * sizeof(float), (size_t)p->n_phase,
+                                         cudaMemcpyDeviceToHost, cs), "D2H slab");
+                }
+            }
+        }
+        cur = dst;
+        dst = (dst == fo_dev) ? buf_ws : fo_dev;
+    }
+    // drain both streams whatever happened, then release the internal objects
+    cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(cs);
+    if (rc == TNLM_OK) { ck(e1, "enhance_host sync"); ck(e2, "enhance_host copy sync"); }
+    for (int s = 0; s < NS; ++s) {
+        if (ev_in[s]) cudaEventDestroy(ev_in[s]);
+        if (ev_out[s]) cudaEventDestroy(ev_out[s]);
+    }
+    if (ev_start) cudaEventDestroy(ev_start);
+    cudaStreamDestroy(cs);
+    return rc;
+}
+
 int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
                       int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream)
 {
@@ -250,6 +326,10 @@ int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_
     float *fi_dev = (float *)((char *)dev_ws + sba);
     float *fo_dev = (float *)((char *)dev_ws + 2 * sba);
     void *ws = (char *)dev_ws + 3 * sba;
+    const int halo = p->search_radius + p->patch_radius;
+    if (!f_init_host && n_iter >= 1 && p->nz >= 32 && p->nz / 4 / 8 * 8 >= halo + 8)
+        return enhance_host_pipelined(p, g_host, f_out_host, n_iter, g_dev, fo_dev, ws, dev_ws_bytes - 3 * sba, st,
+                                      pick_variant(p, TNLM_VARIANT_AUTO));
     cudaError_t e = cudaMemcpyAsync(g_dev, g_host, sb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(e, "H2D g");
     if (f_init_host) {

@@ -241,6 +241,21 @@ def test_enhance_host_matches_device_path(T):
     assert torch.equal(out_h, out_d.cpu())
 
 
+@pytest.mark.parametrize("nz,n_iter,M,d", [(40, 1, 2, 1), (37, 2, 2, 1), (64, 3, 1, 1), (48, 2, 3, 1), (44, 2, 1, 2)])
+def test_enhance_host_pipelined_slabs_bitwise(T, nz, n_iter, M, d):
+    """Volumes of 32+ planes take the pipelined host path (slab-wise H2D / first sweep, last sweep / D2H on a second
+    stream): same bits as the device path, pinned or pageable host memory, and the call may be repeated."""
+    import torch
+    shape = (3, nz, 33, 40)
+    g = random_stack(shape, 70 + nz)
+    p = T.TnlmParams.make(shape, d, M, 0.3, 0.5)
+    want = T.tnlm_enhance(p, dev(g), n_iter).cpu()
+    gh = torch.from_numpy(g).pin_memory()
+    for _ in range(2):
+        assert torch.equal(T.tnlm_enhance_host(p, gh, n_iter), want)
+    assert torch.equal(T.tnlm_enhance_host(p, torch.from_numpy(g), n_iter, f_out_host=torch.empty(shape)), want)
+
+
 def test_device_error_codes(T):
     import torch
     shape = (3, 4, 8, 8)
