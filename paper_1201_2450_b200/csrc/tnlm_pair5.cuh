@@ -39,7 +39,7 @@ template <int M, int RZ, int TX> struct Pair5Geom {
 // CAREFUL as in pair_pass (tnlm_pair.cuh).
 template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE>
 __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
-                                               const float c2, AccPair (&acc)[RZ], const unsigned mask, const bool first = false)
+                                               const float c2, AccPair (&acc)[RZ], const unsigned mask)
 {
     constexpr int NVB = (W + 6) / 2;   // 6 + W - 1 positions
     const float2 nc2 = make_float2(-c2, -c2);
@@ -80,44 +80,43 @@ __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, 
                     const float common = (S.x + S.y) + (u1 + d0);                         // a2y
                     D[q] = add2(make_float2(u0, d1), make_float2(common, common));
                 }
-                if (!CAREFUL || ((mask >> (2 * (p - 4) + i)) & 1u)) {
-                    // `first` (careful form only, warp-uniform): the accumulators are empty and the reference is
-                    // +inf, so the optimistic sum is skipped and the pair goes straight to the re-base
-                    float2 zp = make_float2(INFINITY, INFINITY), np = make_float2(0.f, 0.f);
-                    if (!CAREFUL || !first) {
-                        zp = make_float2(0.f, 0.f);
+                if (!CAREFUL) {
+                    // hot form: optimistic partial sums relative to the reference exponents, one guard per row pair
+                    float2 zp = make_float2(0.f, 0.f), np = make_float2(0.f, 0.f);
 #pragma unroll
-                        for (int q = 0; q < W; ++q) {
-                            const float2 arg = fma2(D[q], nc2, ac.b[i]);                  // a3
-                            const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
-                            zp = add2(zp, u);                                             // a4
-                            np = fma2(u, cand2[i + q], np);
-                        }
+                    for (int q = 0; q < W; ++q) {
+                        const float2 arg = fma2(D[q], nc2, ac.b[i]);                      // a3
+                        const float2 u = make_float2(ex2(arg.x), ex2(arg.y));
+                        zp = add2(zp, u);                                                 // a4
+                        np = fma2(u, cand2[i + q], np);
                     }
                     if (fmaxf(zp.x, zp.y) <= kPairGuard) {
                         ac.z[i] = add2(ac.z[i], zp);
                         ac.n[i] = add2(ac.n[i], np);
-                    } else if (!CAREFUL) {
-                        fail |= 1u << (2 * (p - 4) + i);
                     } else {
-                        float2 dmin = D[0];
-#pragma unroll
-                        for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
-                        // only the row whose partial sum left the band is re-based (the other keeps its reference: sc = 1)
-                        const float2 nb = make_float2(zp.x <= kPairGuard ? ac.b[i].x : fminf(c2 * dmin.x - kPairHead, ac.b[i].x),
-                                                      zp.y <= kPairGuard ? ac.b[i].y : fminf(c2 * dmin.y - kPairHead, ac.b[i].y));
-                        // scale by 2^(nb - b) in two halves: the factor itself may be below 2^-126 when the product is not
-                        const float2 sc = make_float2(ex2(0.5f * (nb.x - ac.b[i].x)), ex2(0.5f * (nb.y - ac.b[i].y)));   // 1 if unchanged, 0 on first use
-                        float2 zz = mul2(mul2(ac.z[i], sc), sc), nn = mul2(mul2(ac.n[i], sc), sc);
-#pragma unroll
-                        for (int q = 0; q < W; ++q) {
-                            const float2 ar = fma2(D[q], nc2, nb);
-                            const float2 u = make_float2(ex2(ar.x), ex2(ar.y));
-                            zz = add2(zz, u);
-                            nn = fma2(u, cand2[i + q], nn);
-                        }
-                        ac.z[i] = zz; ac.n[i] = nn; ac.b[i] = nb;
+                        fail |= 1u << (2 * (p - 4) + i);
                     }
+                } else if ((mask >> (2 * (p - 4) + i)) & 1u) {
+                    // careful form, straight-line: a row is re-based iff its best candidate of this chunk beats its
+                    // reference by more than 2^97 (then the W terms could pass 2^100; on first use the reference is
+                    // +inf); otherwise it keeps its reference (scale factor 1) and its terms are simply added
+                    float2 dmin = D[0];
+#pragma unroll
+                    for (int q = 1; q < W; ++q) dmin = make_float2(fminf(dmin.x, D[q].x), fminf(dmin.y, D[q].y));
+                    const float2 cb = make_float2(c2 * dmin.x, c2 * dmin.y);
+                    const float2 nb = make_float2(ac.b[i].x - cb.x > kPairRebase ? cb.x - kPairHead : ac.b[i].x,
+                                                  ac.b[i].y - cb.y > kPairRebase ? cb.y - kPairHead : ac.b[i].y);
+                    // scale by 2^(nb - b) in two halves: the factor itself may be below 2^-126 when the product is not
+                    const float2 sc = make_float2(ex2(0.5f * (nb.x - ac.b[i].x)), ex2(0.5f * (nb.y - ac.b[i].y)));
+                    float2 zz = mul2(mul2(ac.z[i], sc), sc), nn = mul2(mul2(ac.n[i], sc), sc);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) {
+                        const float2 ar = fma2(D[q], nc2, nb);
+                        const float2 u = make_float2(ex2(ar.x), ex2(ar.y));
+                        zz = add2(zz, u);
+                        nn = fma2(u, cand2[i + q], nn);
+                    }
+                    ac.z[i] = zz; ac.n[i] = nn; ac.b[i] = nb;
                 }
             }
         }
@@ -196,7 +195,7 @@ tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, floa
             constexpr int W = decltype(wtag)::value;
             unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
             if (!first) fail = pair5_pass<RZ, W, false, AP, BP>(aRow, bRow, dm.c2, acc, 0u);
-            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail, first);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail);
         };
 #pragma unroll 1
         for (int k = 0; k < G::E * G::E; ++k) {
