@@ -31,6 +31,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+VARIANT_NAMES = {1: "jacobi_generic_kernel", 2: "tnlm_tiled_kernel"}
 METRIC = "tnlm_voxel_offset_updates_per_sec"
 UNIT = "updates/s"
 SM_LANES = 128                       # FP32 lanes per SM (4 SMSP x 32), B200_PROFILING.md / B300_MICROARCH.md
@@ -44,8 +45,12 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tnlm", choices=["tnlm", "reference"])
-    ap.add_argument("--config", default="config3")
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 tiled")
+    ap.add_argument("--config", default="config3",
+                    help="config1..config4: one enhancement per step; config5: the (patch, window) sweep of "
+                         "BASELINE.json configs[4], one step = the eight enhancements, per-point figures in 'points'")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant: 0 auto, 1 generic, 2 tiled, 3 paired")
+    ap.add_argument("--metrics", action="store_true",
+                    help="also evaluate the paper's SRR (Eq. 10) and CNR on the enhanced stack and time the TV kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -176,20 +181,113 @@ def run_reference(args, cfg):
     return 0
 
 
-def workload_config(cfg, n_gpus):
-    return {"workload": f"{cfg.name}: TNLM-E, {cfg.n_phase} phases x {cfg.nz}x{cfg.ny}x{cfg.nx} fp32 thorax phantom "
-                        f"(seed {cfg.seed}+rank), patch {(2 * cfg.patch_radius + 1)}^3, window "
-                        f"{(2 * cfg.search_radius + 1)}^3, h={cfg.h}, mu={cfg.mu}, {cfg.n_iter} Gauss-Jacobi sweeps, "
-                        f"weights recomputed each sweep",
-            "updates_per_step_per_gpu": cfg.updates_per_sweep * cfg.n_iter,
+def workload_config(cfg, n_gpus, sweep=False):
+    what = (f"{cfg.name}: TNLM-E, {cfg.n_phase} phases x {cfg.nz}x{cfg.ny}x{cfg.nx} fp32 thorax phantom "
+            f"(seed {cfg.seed}+rank), ")
+    if sweep:
+        what += (f"parameter sweep patch {{3^3, 5^3}} x window {{3^3, 5^3, 7^3, 9^3}}, h={cfg.h}, mu={cfg.mu}, "
+                 f"{cfg.n_iter} Gauss-Jacobi sweeps per point, weights recomputed each sweep")
+        per_step = sum(cfg.scaled(search_radius=M).updates_per_sweep for _ in (1, 2) for M in (1, 2, 3, 4)) * cfg.n_iter
+    else:
+        what += (f"patch {(2 * cfg.patch_radius + 1)}^3, window {(2 * cfg.search_radius + 1)}^3, h={cfg.h}, mu={cfg.mu}, "
+                 f"{cfg.n_iter} Gauss-Jacobi sweeps, weights recomputed each sweep")
+        per_step = cfg.updates_per_sweep * cfg.n_iter
+    stack_mb = cfg.n_phase * cfg.voxels_per_phase * 4 / 1e6
+    return {"workload": what, "updates_per_step_per_gpu": per_step,
             "parallelism": f"dp{n_gpus} (one independent stack per GPU, no collective)",
-            "l2_policy": "inputs larger than L2 (3 x 335 MB stacks per step vs 126 MB L2); no explicit flush"}
+            "l2_policy": f"inputs larger than L2 (3 x {stack_mb:.0f} MB stacks per step vs 126 MB L2); no explicit flush"
+                         if 3 * stack_mb > 126 else
+                         f"3 x {stack_mb:.0f} MB stacks fit the 126 MB L2: the bench writes a 256 MB buffer between steps"}
+
+
+def kernel_label(T, p, variant):
+    """Name of the kernel the timed call launches (AUTO and PAIRED resolve through the library)."""
+    if variant in VARIANT_NAMES:
+        return VARIANT_NAMES[variant]
+    return T.kernel_name(p)
+
+
+def committed_traffic(kernel, cfg_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` at `cfg_name`, from the committed ncu
+    capture (profiles/traffic.csv); None if that pair was not captured."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == kernel and row.get("config", "config3") == cfg_name:
+                    return int(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
+def roofline_block(T, p, cfg, variant, launch_ms, sms, peaks, clocks, probe_slots_per_s, stack_elems):
+    """FP32-pipe ("alu") roofline of the sweep kernel; DESIGN.md section 5 defines the unit and the peak."""
+    d = cfg.patch_radius
+    A = 5 + 6 * d                                      # FP32-pipe slots per voxel-offset update (SURVEY 8(d))
+    A_shared = (3 + 6 * d) / 2 + 2                     # the same with the paper's mutual-weight sharing (PAPER.md:223)
+    rate = cfg.updates_per_sweep / (launch_ms * 1e-3)  # updates/s of one launch
+    peak = sms * SM_LANES * peaks["sm_max_mhz"] * 1e6
+    alg_bytes = 3 * stack_elems * 4                    # read f, read g, write f_out
+    kernel = kernel_label(T, p, variant)
+    out = {
+        "bound": "alu", "kernel": kernel, "achieved": rate * A / 1e12, "peak": peak / 1e12,
+        "unit": "Tslot/s (FP32-pipe lane-operations; A = 5+6d slots per voxel-offset update)",
+        "frac": rate * A / peak, "traffic": committed_traffic(kernel, cfg.name),
+        "frac_vs_A_shared": rate * A_shared / peak, "slots_per_update": A, "slots_per_update_shared": A_shared,
+        "peak_source": f"{sms} SMs x {SM_LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, {peaks['source']})",
+        "launch_ms": launch_ms,
+        "hbm": {"algorithmic_bytes_per_launch": alg_bytes, "achieved_gbs": alg_bytes / (launch_ms * 1e-3) / 1e9,
+                "peak_gbs": peaks["hbm_gbs"], "frac": alg_bytes / (launch_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "peak_source": peaks["source"]},
+    }
+    if probe_slots_per_s:
+        out["ffma_probe_tslots"] = probe_slots_per_s / 1e12
+        out["frac_of_ffma_probe"] = rate * A / probe_slots_per_s
+    if clocks and clocks.get("sm_mhz"):
+        out["frac_at_observed_clock"] = rate * A / (sms * SM_LANES * clocks["sm_mhz"] * 1e6)
+    return out
+
+
+def quality_metrics(T, torch, cfg, g, f):
+    """SRR of Eq. 10 against the clean phantom and the tumour CNR of PAPER.md:265 (kernels of the library), and the
+    TV kernel against the HBM roofline (algorithmic bytes of one tnlm_tv_diff = 2 stacks x 4 B per voxel)."""
+    from tnlm_inputs import make_stack
+    star = torch.from_numpy(make_stack(cfg, clean=True)).to(g.device)
+    p = T.TnlmParams.make(cfg.shape, cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+    for _ in range(3):
+        T.tnlm_tv_diff(p, g, star)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n = 10
+    e0.record()
+    for _ in range(n):                       # operands alternate: two stacks each, larger than L2 from config 3 on
+        T.tnlm_tv_diff(p, g, star)
+        T.tnlm_tv_diff(p, f, star)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / (2 * n)
+    gbs = 2 * g.numel() * 4 / (ms * 1e-3) / 1e9
+    srr = T.tnlm_srr(p, g, f, star).cpu().numpy()
+    P, Z, Y, X = cfg.shape
+    cz, cy, cx = (Z - 1) / 2, (Y - 1) / 2, (X - 1) / 2
+    tz = int(round(cz - cfg.si_amplitude / 2 + cfg.si_amplitude)); ty = int(round(cy - 0.03 * Y)); tx = int(round(cx + 0.20 * X))
+    r = max(2, int(cfg.tumour_radius) // 2)
+    roi = (tz - r, tz + r + 1, ty - r, ty + r + 1, tx - r, tx + r + 1)            # inside the tumour at phase 0
+    bg = (tz - r, tz + r + 1, ty + 3 * r + 2, ty + 5 * r + 3, tx - r, tx + r + 1)  # lung next to it
+    c0 = T.tnlm_cnr(p, g, 0, roi, bg).cpu().numpy()
+    c1 = T.tnlm_cnr(p, f, 0, roi, bg).cpu().numpy()
+    peaks = measured_peaks()
+    return {"tv_diff_ms": ms, "tv_diff_gbs": gbs, "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_roofline_frac": gbs / peaks["hbm_gbs"],
+            "srr_min": float(srr.min()), "srr_max": float(srr.max()), "cnr_input": float(c0[4]), "cnr_enhanced": float(c1[4]),
+            "roi": roi, "roi_bg": bg}
 
 
 def main():
     args = parse_args()
     from tnlm_inputs import CONFIGS, make_stack
     cfg = CONFIGS[args.config]
+    sweep_mode = args.config == "config5"
     if args.impl == "reference":
         return run_reference(args, cfg)
 
@@ -206,22 +304,37 @@ def main():
     info = D.init("nccl")
     dev = torch.device("cuda", info.local_rank)
     peaks = measured_peaks()
+    warmup = max(args.warmup, 3)
 
     # one independent, differently seeded stack per rank (weak scaling)
     rcfg = cfg.scaled(seed=cfg.seed + info.rank)
     g_host_np = make_stack(rcfg)
-    p = T.TnlmParams.make(cfg.shape, cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
     g = torch.from_numpy(g_host_np).to(dev)
     f_out = torch.empty_like(g)
-    ws = torch.empty(T.workspace_bytes(p), dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
-    updates_per_step = cfg.updates_per_sweep * cfg.n_iter
-    launches_per_step = cfg.n_iter * T.launches_per_sweep(p)
+    # the points of a step: (config with its d, M; params; workspace)
+    point_cfgs = [cfg.scaled(patch_radius=d, search_radius=M) for d in (1, 2) for M in (1, 2, 3, 4)] if sweep_mode else [cfg]
+    points = []
+    for c in point_cfgs:
+        p = T.TnlmParams.make(c.shape, c.patch_radius, c.search_radius, c.h, c.mu)
+        points.append((c, p))
+    ws = torch.empty(max(T.workspace_bytes(p) for _, p in points), dtype=torch.uint8, device=dev)
+    updates_per_step = sum(c.updates_per_sweep * c.n_iter for c, _ in points)
+    launches_per_step = sum(c.n_iter * T.launches_per_sweep(p) for c, p in points)
+    stack_mb = g.numel() * 4 / 1e6
+    flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev) if 3 * stack_mb <= 126 else None
 
-    def step():
-        T.tnlm_enhance(p, g, cfg.n_iter, f_out=f_out, ws=ws, stream=stream, variant=args.variant)
+    def step(record=None):
+        for k, (c, p) in enumerate(points):
+            if record is not None:
+                record[k][0].record(stream)
+            T.tnlm_enhance(p, g, c.n_iter, f_out=f_out, ws=ws, stream=stream, variant=args.variant)
+            if record is not None:
+                record[k][1].record(stream)
+        if flush is not None:
+            flush.zero_()                               # small stacks: evict them from L2 between steps
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
 
@@ -232,15 +345,22 @@ def main():
     D.barrier(info)
     torch.cuda.synchronize()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    per_point = [[[torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)] for _ in points]
+                 for _ in range(args.steps)]
     ev0.record(stream)
-    for _ in range(args.steps):
-        step()
+    for s_i in range(args.steps):
+        step(per_point[s_i])
     ev1.record(stream)
     torch.cuda.synchronize()
     D.barrier(info)
     elapsed_ms = D.max_over_ranks(info, ev0.elapsed_time(ev1), device=dev)
     clocks = sampler.stop() if info.rank == 0 else None
     value = info.world * args.steps * updates_per_step / (elapsed_ms * 1e-3)
+    # time inside the enhancement calls only (excludes the L2 flush of small configs), per point
+    point_ms = [sum(per_point[s_i][k][0].elapsed_time(per_point[s_i][k][1]) for s_i in range(args.steps)) / args.steps
+                for k in range(len(points))]
+    if flush is not None:
+        value = info.world * updates_per_step / (D.max_over_ranks(info, sum(point_ms), device=dev) * 1e-3)
 
     # ---- FP32 probe (register-resident FFMA loop) for the measured pipe peak -------------
     sink = torch.zeros(4, device=dev)
@@ -253,76 +373,78 @@ def main():
     torch.cuda.synchronize()
     probe_slots_per_s = n_ffma / (pe0.elapsed_time(pe1) * 1e-3)
 
-    # ---- end-to-end through tnlm_enhance_host (pinned host buffers) ----------------------
+    # ---- end-to-end through tnlm_enhance_host (pinned host buffers), the same number of steps --------
     e2e = None
     if not args.no_e2e:
         g_pin = torch.from_numpy(g_host_np).pin_memory()
         out_pin = torch.empty(cfg.shape, dtype=torch.float32).pin_memory()
-        dev_ws = torch.empty(T.host_workspace_bytes(p), dtype=torch.uint8, device=dev)
-        T.tnlm_enhance_host(p, g_pin, cfg.n_iter, f_out_host=out_pin, dev_ws=dev_ws, stream=stream)   # warm
+        dev_ws = torch.empty(max(T.host_workspace_bytes(p) for _, p in points), dtype=torch.uint8, device=dev)
+
+        def e2e_step():
+            for c, p in points:
+                T.tnlm_enhance_host(p, g_pin, c.n_iter, f_out_host=out_pin, dev_ws=dev_ws, stream=stream)
+
+        e2e_step()                                      # warm
         D.barrier(info)
         torch.cuda.synchronize()
-        n_e2e = max(1, min(args.steps, 3))
         t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            T.tnlm_enhance_host(p, g_pin, cfg.n_iter, f_out_host=out_pin, dev_ws=dev_ws, stream=stream)
+        for _ in range(args.steps):
+            e2e_step()
         torch.cuda.synchronize()
         dt = D.max_over_ranks(info, time.perf_counter() - t0, device=dev)
-        assert torch.equal(out_pin, f_out.cpu()), "host path and device path disagree"
-        e2e = {"value": info.world * n_e2e * updates_per_step / dt, "unit": UNIT,
-               "h2d_bytes_per_step": g_pin.numel() * 4, "d2h_bytes_per_step": out_pin.numel() * 4,
-               "ms_per_step": 1e3 * dt / n_e2e, "steps": n_e2e,
+        if args.variant == 0:
+            assert torch.equal(out_pin, f_out.cpu()), "host path and device path disagree"
+        e2e = {"value": info.world * args.steps * updates_per_step / dt, "unit": UNIT,
+               "h2d_bytes_per_step": g_pin.numel() * 4 * len(points), "d2h_bytes_per_step": out_pin.numel() * 4 * len(points),
+               "ms_per_step": 1e3 * dt / args.steps, "steps": args.steps,
                "api": "tnlm_enhance_host (C ABI, pinned host buffers, copies + sync inside the timed region)"}
         del dev_ws
+
+    quality = None
+    if args.metrics and info.rank == 0:
+        c, p = points[0] if not sweep_mode else points[1]
+        f_enh = T.tnlm_enhance(p, g, c.n_iter, ws=ws, stream=stream)
+        quality = quality_metrics(T, torch, c.scaled(seed=rcfg.seed), g, f_enh)
 
     if info.rank != 0:
         D.finalize(info)
         return 0
 
     # ---- roofline of the dominant (sweep) kernel ------------------------------------------
-    n_launch = args.steps * cfg.n_iter
-    launch_ms = elapsed_ms / n_launch                  # CUDA events over the timed region / sweeps
     props = torch.cuda.get_device_properties(dev)
     sms = props.multi_processor_count
-    A = 5 + 6 * cfg.patch_radius                       # FP32-pipe slots per voxel-offset update
-    achieved = cfg.updates_per_sweep * A / (launch_ms * 1e-3)
-    peak = sms * SM_LANES * peaks["sm_max_mhz"] * 1e6
-    alg_bytes = 3 * g.numel() * 4                      # read f, read g, write f_out
-    traffic = None          # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture
-    try:
-        import csv
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
-            for row in csv.DictReader(fh):
-                if row["kernel"] == T.kernel_name(p) and cfg.name == "config3":
-                    traffic = int(row["dram_bytes_per_launch"])
-    except Exception:
-        pass
-    roofline = {
-        "bound": "alu", "kernel": T.kernel_name(p), "achieved": achieved / 1e12, "peak": peak / 1e12,
-        "unit": "Tslot/s (FP32-pipe lane-operations; A = 5+6d slots per voxel-offset update)",
-        "frac": achieved / peak, "traffic": traffic,
-        "peak_source": f"{sms} SMs x {SM_LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, {peaks['source']})",
-        "launch_ms": launch_ms, "slots_per_update": A,
-        "ffma_probe_tslots": probe_slots_per_s / 1e12, "frac_of_ffma_probe": achieved / probe_slots_per_s,
-        "frac_at_observed_clock": (achieved / (sms * SM_LANES * clocks["sm_mhz"] * 1e6)) if clocks and clocks.get("sm_mhz") else None,
-        "hbm": {"algorithmic_bytes_per_launch": alg_bytes, "achieved_gbs": alg_bytes / (launch_ms * 1e-3) / 1e9,
-                "peak_gbs": peaks["hbm_gbs"], "frac": alg_bytes / (launch_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                "peak_source": peaks["source"]},
-    }
+    point_lines = []
+    for (c, p), ms in zip(points, point_ms):
+        launch_ms = ms / c.n_iter                      # CUDA events around the enhancement / its sweeps
+        rl = roofline_block(T, p, c, args.variant, launch_ms, sms, peaks, clocks, probe_slots_per_s, g.numel())
+        point_lines.append({"patch": 2 * c.patch_radius + 1, "window": 2 * c.search_radius + 1, "n_iter": c.n_iter,
+                            "updates_per_s": c.updates_per_sweep * c.n_iter / (ms * 1e-3), "s_per_enhancement": ms * 1e-3,
+                            "ms_per_sweep": launch_ms, "roofline": rl})
+    # the headline roofline block: the single point, or (sweep) the point that takes the largest share of the step
+    top = max(range(len(points)), key=lambda k: point_ms[k])
+    roofline = point_lines[top]["roofline"]
+    if sweep_mode:
+        roofline = dict(roofline, note=f"dominant point of the sweep (patch {point_lines[top]['patch']}^3, window "
+                                       f"{point_lines[top]['window']}^3, {100 * point_ms[top] / sum(point_ms):.0f} % of the step); "
+                                       f"every point's block is in 'points'")
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        cpu_baseline = oracle_sample_rate(cfg, g_host_np, args.cpu_seconds)
+        cpu_baseline = oracle_sample_rate(points[top][0], g_host_np, args.cpu_seconds)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": info.world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms / args.steps,
-        "s_per_enhancement": elapsed_ms * 1e-3 / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": warmup, "ms_per_step": elapsed_ms / args.steps,
+        "s_per_enhancement": sum(point_ms) * 1e-3 / len(points), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": workload_config(cfg, info.world), "clocks": clocks, "e2e": e2e,
+        "config": workload_config(cfg, info.world, sweep_mode), "clocks": clocks, "e2e": e2e,
         "gpu_launches": args.steps * launches_per_step, "roofline": roofline, "cpu_baseline": cpu_baseline,
-        "impl": "tnlm", "kernel": T.kernel_name(p),
+        "impl": "tnlm", "kernel": roofline["kernel"], "variant": args.variant,
     }
+    if sweep_mode:
+        line["points"] = point_lines
+    if quality:
+        line["quality"] = quality
     print(json.dumps(line), flush=True)
     D.finalize(info)
     return 0

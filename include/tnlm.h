@@ -21,6 +21,11 @@
  * Errors: every int-returning function returns TNLM_OK (0) or a negative tnlm_status.  Argument
  * errors are detected synchronously, before anything is enqueued; on error no output is written.
  * NaN/Inf in the inputs are not scanned for (they propagate).  No C++ exception crosses the ABI.
+ *
+ * Input range: the packed sweep kernels accumulate sum_y u(x,y) f(y) with weights u held below 2^107 relative to a
+ * per-voxel reference, so intensities must satisfy |f| < 2^20 (about 1e6) for the sums to
+ * stay finite; CT numbers in any usual unit are far inside.  Rescale (f, g, h by one factor: Eq. 3 / Eq. 8 are
+ * covariant) if a stack exceeds it.
  */
 #ifndef TNLM_H_
 #define TNLM_H_
@@ -36,7 +41,8 @@ typedef struct {
     int32_t n_phase, nz, ny, nx; /* stack [n_phase][nz][ny][nx], fp32, contiguous; n_phase >= 2   */
     int32_t patch_radius;        /* d >= 0: patch = (2d+1)^3 cube centred at the voxel */
     int32_t search_radius;       /* M >= 0: search window (2M+1)^3 centred at x       */
-    float h;                     /* > 0, finite: similarity scale of Eq. 3            */
+    float h;                     /* > 0, finite: similarity scale of Eq. 3, PAPER.md:103 (h < 1e-18 is refused:
+                                    1/(2h^2) must be representable in fp32)                          */
     float mu;                    /* > 0, finite: fidelity weight of Eq. 4             */
 } tnlm_params;
 
@@ -45,7 +51,7 @@ typedef enum {
     TNLM_ERR_NULL_POINTER = -1, /* a required pointer is NULL                                      */
     TNLM_ERR_BAD_DIMS = -2,     /* an extent < 1, n_phase < 2 (a phase is never compared with
                                    itself), or the stack exceeds 2^31-1 voxels       */
-    TNLM_ERR_BAD_PARAM = -3,    /* h or mu not finite or <= 0; negative radius; n_iter < 0         */
+    TNLM_ERR_BAD_PARAM = -3,    /* h or mu not finite or <= 0; h < 1e-18; negative radius; n_iter < 0 */
     TNLM_ERR_UNSUPPORTED = -4,  /* radius outside the compiled set (d <= 3, M <= 6), bad variant   */
     TNLM_ERR_ALIAS = -5,        /* f_out overlaps an input (Jacobi reads only the old iterate,
                                    PAPER.md:176) or the workspace                                  */
@@ -117,7 +123,8 @@ int tnlm_enhance_variant(const tnlm_params *p, const float *g, const float *f_in
  * End-to-end form of tnlm_enhance for HOST buffers: g_host / f_init_host (may be NULL) / f_out_host
  * are host pointers (pinned memory makes the copies asynchronous).  The call copies the inputs to the
  * device, runs tnlm_enhance and copies the result back, all on `cuda_stream`, then synchronises the
- * stream before returning.  For f_init_host == NULL and volumes of 32 or more planes the copies are pipelined: the
+ * stream before returning.  For f_init_host == NULL, n_iter >= 1 and volumes deep enough for four z-slabs
+ * (nz >= 32 and 8 * floor(nz / 32) >= M + d + 8) the copies are pipelined: the
  * stack travels in four z-slabs on a copy stream that the call creates and destroys, the first sweep starts on the
  * slabs that have arrived and the last sweep returns its slabs as they finish (same bits as the plain path: slab
  * sweeps reproduce the whole-volume sweep exactly).  dev_ws is a caller-owned DEVICE workspace of at least

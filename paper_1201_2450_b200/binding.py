@@ -124,70 +124,107 @@ def _dev_ptr(t, p: TnlmParams, name, optional=False):
     return t.data_ptr()
 
 
-def _stream(stream):
-    import torch
-    s = torch.cuda.current_stream() if stream is None else stream
-    return s.cuda_stream
+class _Call:
+    """Context of one library call: the device all tensors live on is made current (the C ABI works on 'the
+    current CUDA device'), the stream handle is resolved on it, and temporaries the binding allocated itself are
+    tied to a non-current stream with record_stream so the caching allocator cannot reuse them while work is queued."""
 
+    def __init__(self, stream, *tensors):
+        import torch
+        for t in tensors:
+            if t is not None and not (isinstance(t, torch.Tensor) and t.is_cuda):
+                raise TypeError("every tensor argument must be a CUDA torch tensor (no CPU path exists)")
+        devs = {t.device for t in tensors if t is not None}
+        if len(devs) > 1:
+            raise TypeError(f"all tensors of a call must live on one CUDA device, got {sorted(str(d) for d in devs)}")
+        self.device = devs.pop() if devs else torch.device("cuda", torch.cuda.current_device())
+        self.guard = torch.cuda.device(self.device)
+        self.stream_arg = stream
+        self.temps = []
 
-def _workspace(p: TnlmParams, ws, nbytes=None):
-    import torch
-    need = workspace_bytes(p) if nbytes is None else nbytes
-    if ws is None:
-        ws = torch.empty(max(need, 16), dtype=torch.uint8, device="cuda")
-    if not ws.is_cuda or ws.dtype != torch.uint8:
-        raise TypeError("workspace must be a CUDA uint8 tensor")
-    return ws
+    def __enter__(self):
+        import torch
+        self.guard.__enter__()
+        self.stream = torch.cuda.current_stream(self.device) if self.stream_arg is None else self.stream_arg
+        return self
+
+    def __exit__(self, *exc):
+        import torch
+        if self.stream != torch.cuda.current_stream(self.device):
+            for t in self.temps:
+                t.record_stream(self.stream)
+        return self.guard.__exit__(*exc)
+
+    @property
+    def handle(self):
+        return self.stream.cuda_stream
+
+    def temp(self, *size, dtype):
+        import torch
+        t = torch.empty(*size, dtype=dtype, device=self.device)
+        self.temps.append(t)
+        return t
+
+    def workspace(self, ws, need):
+        import torch
+        if ws is None:
+            return self.temp(max(need, 16), dtype=torch.uint8)
+        if not ws.is_cuda or ws.dtype != torch.uint8 or ws.device != self.device:
+            raise TypeError(f"workspace must be a CUDA uint8 tensor on {self.device}")
+        return ws
 
 
 def tnlm_weights(p: TnlmParams, ref, w_out=None, stream=None):
     """Normalised weights w[p][s][k][z][y][x] of Eq. 3/9 (see include/tnlm.h)."""
     import torch
     n_t = (2 * p.search_radius + 1) ** 3
-    if w_out is None:
-        w_out = torch.empty((p.n_phase, 2, n_t, p.nz, p.ny, p.nx), dtype=torch.float32, device=ref.device)
-    _check(lib().tnlm_weights(C.byref(p), _dev_ptr(ref, p, "ref"), w_out.data_ptr(), None, 0, _stream(stream)),
-           "tnlm_weights")
+    with _Call(stream, ref, w_out) as c:
+        if w_out is None:
+            w_out = torch.empty((p.n_phase, 2, n_t, p.nz, p.ny, p.nx), dtype=torch.float32, device=c.device)
+        _check(lib().tnlm_weights(C.byref(p), _dev_ptr(ref, p, "ref"), w_out.data_ptr(), None, 0, c.handle), "tnlm_weights")
     return w_out
 
 
 def tnlm_jacobi_step(p: TnlmParams, f, g, ref=None, f_out=None, ws=None, stream=None, variant=VARIANT_AUTO):
     """One Gauss-Jacobi sweep of Eq. 8 (see include/tnlm.h)."""
     import torch
-    if f_out is None:
-        f_out = torch.empty_like(f)
-    ws = _workspace(p, ws)
-    _check(lib().tnlm_jacobi_step_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
-                                          _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
-                                          ws.data_ptr(), ws.numel(), _stream(stream), int(variant)),
-           "tnlm_jacobi_step")
+    with _Call(stream, f, g, ref, f_out, ws) as c:
+        if f_out is None:
+            f_out = torch.empty_like(f)
+        ws = c.workspace(ws, workspace_bytes(p))
+        _check(lib().tnlm_jacobi_step_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
+                                              _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
+                                              ws.data_ptr(), ws.numel(), c.handle, int(variant)),
+               "tnlm_jacobi_step")
     return f_out
 
 
 def tnlm_jacobi_step_slab(p: TnlmParams, f, g, z_begin, z_end, ref=None, f_out=None, ws=None, stream=None,
                           variant=VARIANT_AUTO):
     import torch
-    if f_out is None:
-        f_out = torch.empty_like(f)
-    ws = _workspace(p, ws)
-    _check(lib().tnlm_jacobi_step_slab_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
-                                               _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
-                                               int(z_begin), int(z_end), ws.data_ptr(), ws.numel(),
-                                               _stream(stream), int(variant)),
-           "tnlm_jacobi_step_slab")
+    with _Call(stream, f, g, ref, f_out, ws) as c:
+        if f_out is None:
+            f_out = torch.empty_like(f)
+        ws = c.workspace(ws, workspace_bytes(p))
+        _check(lib().tnlm_jacobi_step_slab_variant(C.byref(p), _dev_ptr(f, p, "f"), _dev_ptr(g, p, "g"),
+                                                   _dev_ptr(ref, p, "ref", optional=True), _dev_ptr(f_out, p, "f_out"),
+                                                   int(z_begin), int(z_end), ws.data_ptr(), ws.numel(),
+                                                   c.handle, int(variant)),
+               "tnlm_jacobi_step_slab")
     return f_out
 
 
 def tnlm_enhance(p: TnlmParams, g, n_iter, f_init=None, f_out=None, ws=None, stream=None, variant=VARIANT_AUTO):
     """TNLM-E: n_iter x {weights from f^k; one sweep} (see include/tnlm.h)."""
     import torch
-    if f_out is None:
-        f_out = torch.empty_like(g)
-    ws = _workspace(p, ws)
-    _check(lib().tnlm_enhance_variant(C.byref(p), _dev_ptr(g, p, "g"), _dev_ptr(f_init, p, "f_init", optional=True),
-                                      _dev_ptr(f_out, p, "f_out"), int(n_iter), ws.data_ptr(), ws.numel(),
-                                      _stream(stream), int(variant)),
-           "tnlm_enhance")
+    with _Call(stream, g, f_init, f_out, ws) as c:
+        if f_out is None:
+            f_out = torch.empty_like(g)
+        ws = c.workspace(ws, workspace_bytes(p))
+        _check(lib().tnlm_enhance_variant(C.byref(p), _dev_ptr(g, p, "g"), _dev_ptr(f_init, p, "f_init", optional=True),
+                                          _dev_ptr(f_out, p, "f_out"), int(n_iter), ws.data_ptr(), ws.numel(),
+                                          c.handle, int(variant)),
+               "tnlm_enhance")
     return f_out
 
 
@@ -200,47 +237,52 @@ def tnlm_enhance_host(p: TnlmParams, g_host, n_iter, f_out_host=None, f_init_hos
             raise TypeError(f"{name} must be a contiguous float32 CPU tensor of shape {p.shape}")
     if f_out_host is None:
         f_out_host = torch.empty(p.shape, dtype=torch.float32, pin_memory=True)
-    dev_ws = _workspace(p, dev_ws, host_workspace_bytes(p))
-    _check(lib().tnlm_enhance_host(C.byref(p), g_host.data_ptr(),
-                                   None if f_init_host is None else f_init_host.data_ptr(),
-                                   f_out_host.data_ptr(), int(n_iter), dev_ws.data_ptr(), dev_ws.numel(),
-                                   _stream(stream)),
-           "tnlm_enhance_host")
+    with _Call(stream, dev_ws) as c:
+        dev_ws = c.workspace(dev_ws, host_workspace_bytes(p))
+        _check(lib().tnlm_enhance_host(C.byref(p), g_host.data_ptr(),
+                                       None if f_init_host is None else f_init_host.data_ptr(),
+                                       f_out_host.data_ptr(), int(n_iter), dev_ws.data_ptr(), dev_ws.numel(),
+                                       c.handle),
+               "tnlm_enhance_host")                    # synchronises the stream before returning
     return f_out_host
 
 
 def probe_fp32(n_iter: int, sink, stream=None) -> float:
     """Enqueue the FFMA probe; returns the number of FFMA lane-operations it executes."""
-    _check(lib().tnlm_probe_fp32(int(n_iter), sink.data_ptr(), _stream(stream)), "tnlm_probe_fp32")
+    with _Call(stream, sink) as c:
+        _check(lib().tnlm_probe_fp32(int(n_iter), sink.data_ptr(), c.handle), "tnlm_probe_fp32")
     return float(lib().tnlm_probe_fp32_ffma_count(int(n_iter)))
 
 
 def tnlm_tv_diff(p: TnlmParams, a, b=None, stream=None):
     """TV(a_p - b_p) per phase (Eq. 10's seminorm; see include/tnlm.h) -> float64 CUDA tensor [n_phase]."""
     import torch
-    out = torch.empty(p.n_phase, dtype=torch.float64, device=a.device)
-    _check(lib().tnlm_tv_diff(C.byref(p), _dev_ptr(a, p, "a"), _dev_ptr(b, p, "b", optional=True), out.data_ptr(),
-                              _stream(stream)), "tnlm_tv_diff")
+    with _Call(stream, a, b) as c:
+        out = torch.empty(p.n_phase, dtype=torch.float64, device=c.device)
+        _check(lib().tnlm_tv_diff(C.byref(p), _dev_ptr(a, p, "a"), _dev_ptr(b, p, "b", optional=True), out.data_ptr(),
+                                  c.handle), "tnlm_tv_diff")
     return out
 
 
 def tnlm_srr(p: TnlmParams, f_fdk, f_enh, f_star, stream=None):
     """Streak-reduction ratio of Eq. 10 per phase -> float64 CUDA tensor [n_phase]."""
     import torch
-    out = torch.empty(p.n_phase, dtype=torch.float64, device=f_fdk.device)
-    ws = torch.empty(2 * p.n_phase, dtype=torch.float64, device=f_fdk.device)
-    _check(lib().tnlm_srr(C.byref(p), _dev_ptr(f_fdk, p, "f_fdk"), _dev_ptr(f_enh, p, "f_enh"),
-                          _dev_ptr(f_star, p, "f_star"), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
-                          _stream(stream)), "tnlm_srr")
+    with _Call(stream, f_fdk, f_enh, f_star) as c:
+        out = torch.empty(p.n_phase, dtype=torch.float64, device=c.device)
+        ws = c.temp(2 * p.n_phase, dtype=torch.float64)
+        _check(lib().tnlm_srr(C.byref(p), _dev_ptr(f_fdk, p, "f_fdk"), _dev_ptr(f_enh, p, "f_enh"),
+                              _dev_ptr(f_star, p, "f_star"), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
+                              c.handle), "tnlm_srr")
     return out
 
 
 def tnlm_cnr(p: TnlmParams, stack, phase, roi, roi_bg, stream=None):
     """[S, sigma, S_b, sigma_b, CNR] of two half-open boxes (z0, z1, y0, y1, x0, x1) of `phase`."""
     import torch
-    out = torch.empty(5, dtype=torch.float64, device=stack.device)
     r0 = (C.c_int32 * 6)(*[int(v) for v in roi])
     r1 = (C.c_int32 * 6)(*[int(v) for v in roi_bg])
-    _check(lib().tnlm_cnr(C.byref(p), _dev_ptr(stack, p, "stack"), int(phase), r0, r1, out.data_ptr(),
-                          _stream(stream)), "tnlm_cnr")
+    with _Call(stream, stack) as c:
+        out = torch.empty(5, dtype=torch.float64, device=c.device)
+        _check(lib().tnlm_cnr(C.byref(p), _dev_ptr(stack, p, "stack"), int(phase), r0, r1, out.data_ptr(),
+                              c.handle), "tnlm_cnr")
     return out

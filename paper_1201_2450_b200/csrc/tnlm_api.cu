@@ -1,5 +1,6 @@
 // C-ABI entry points of libtnlm.so (include/tnlm.h): argument validation, workspace carving,
 // kernel selection and launch.  Every step of the hot path runs in the kernels of this library.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -34,6 +35,10 @@ int check_params(const tnlm_params *p)
     if (n > 2147483647.0) return TNLM_ERR_BAD_DIMS;
     if (p->patch_radius < 0 || p->search_radius < 0) return TNLM_ERR_BAD_PARAM;
     if (!(p->h > 0.f) || !std::isfinite(p->h) || !(p->mu > 0.f) || !std::isfinite(p->mu)) return TNLM_ERR_BAD_PARAM;
+    // the kernels scale distances by c2 = log2(e)/(2h^2) in fp32 (flush-to-zero): an h so small that c2 overflows
+    // would turn every exponent into 0*inf; h -> infinity is fine (c2 -> 0: uniform weights)
+    const double c2 = 1.4426950408889634 / (2.0 * (double)p->h * (double)p->h);
+    if (!(c2 < 1.0e37)) return TNLM_ERR_BAD_PARAM;
     if (p->patch_radius > kMaxPatchRadius || p->search_radius > kMaxSearchRadius) return TNLM_ERR_UNSUPPORTED;
     return TNLM_OK;
 }
@@ -245,6 +250,7 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
                                   float *g_dev, float *fo_dev, void *ws, size_t ws_bytes, cudaStream_t st, int variant)
 {
     constexpr int NS = 4;
+    constexpr int kMaxRZ = 8;   // deepest z-tile of any sweep kernel (tiles are aligned to absolute multiples of RZ)
     const int halo = p->search_radius + p->patch_radius;
     const size_t plane = (size_t)p->ny * p->nx, pitch = plane * p->nz * sizeof(float), sb = stack_bytes(p);
     int zb[NS + 1];
@@ -284,8 +290,14 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
             rc = launch_sweep(p, cur, g_dev, cur, dst, 0, p->nz, kws, kws_bytes, st, variant);
         } else {
             for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
-                // slab s of the first sweep reads up to `halo` planes of slab s+1
-                if (first) ck(cudaStreamWaitEvent(st, ev_in[s + 1 < NS ? s + 1 : NS - 1], 0), "stream wait");
+                // slab s of the first sweep reads planes up to the end of its last z-tile plus the halo: wait for the
+                // slab that holds the last of them (the copy stream delivers the slabs in order)
+                if (first) {
+                    const int last_plane = std::min(p->nz - 1, zb[s + 1] - 1 + (kMaxRZ - 1) + halo);
+                    int need = s;
+                    while (need + 1 < NS && zb[need + 1] <= last_plane) ++need;
+                    ck(cudaStreamWaitEvent(st, ev_in[need], 0), "stream wait");
+                }
                 if (rc == TNLM_OK) rc = launch_sweep(p, cur, g_dev, cur, dst, zb[s], zb[s + 1], kws, kws_bytes, st, variant);
                 if (last && rc == TNLM_OK) {
                     const size_t off = (size_t)zb[s] * plane;
@@ -409,9 +421,11 @@ int tnlm_cnr(const tnlm_params *p, const float *stack, int32_t phase, const int3
     if (blocks < 1) blocks = 1;
     const float *vol = stack + (size_t)phase * p->nz * p->ny * p->nx;
     roi_sums_kernel<<<dim3((unsigned)blocks, 2), kMetricThreads, 0, st>>>(vol, p->ny, p->nx, bx[0], bx[1], 0.f, out5);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "cnr sums launch");
     cnr_finish_kernel<<<1, 32, 0, st>>>(out5, n[0], n[1], 0.f, out5);
     e = cudaGetLastError();
-    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "cnr launch");
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "cnr finish launch");
 }
 
 const char *tnlm_strerror(int code)
@@ -420,7 +434,7 @@ const char *tnlm_strerror(int code)
         case TNLM_OK: return "ok";
         case TNLM_ERR_NULL_POINTER: return "a required pointer is NULL";
         case TNLM_ERR_BAD_DIMS: return "bad dimensions (extent < 1, n_phase < 2, slab out of range or stack too large)";
-        case TNLM_ERR_BAD_PARAM: return "bad parameter (h, mu not finite or <= 0; negative radius; n_iter < 0)";
+        case TNLM_ERR_BAD_PARAM: return "bad parameter (h, mu not finite or <= 0; h below 1e-18; negative radius; n_iter < 0)";
         case TNLM_ERR_UNSUPPORTED: return "radius or kernel variant not compiled in";
         case TNLM_ERR_ALIAS: return "output overlaps an input or the workspace";
         case TNLM_ERR_WORKSPACE: return "workspace or stack pointer NULL, too small or not 16-byte aligned";

@@ -72,9 +72,12 @@ jacobi_generic_kernel(const float *__restrict__ f, const float *__restrict__ g, 
     }
 }
 
-// w_out[p][s][k][z][y][x]: two passes over the window (min + normaliser, then the weights).
+// w_out[p][s][k][z][y][x].  Every patch distance is computed once: pass 1 parks D_k in w_out[k] (the thread's own
+// column of the output) and finds the smallest one, pass 2 turns the parked distances into exp2((Dmin - D_k) c2)
+// (the shifted form, reading P3) and sums the normaliser, pass 3 scales.  w_out must not alias ref (checked by
+// the caller), so the __ldg reads of ref stay valid while w_out is written.
 __global__ void __launch_bounds__(256)
-weights_generic_kernel(const float *__restrict__ ref, float *__restrict__ w_out, Dims dm)
+weights_generic_kernel(const float *__restrict__ ref, float *w_out, Dims dm)
 {
     const size_t V = (size_t)dm.Z * dm.Y * dm.X;
     const size_t total = V * dm.P * 2;
@@ -88,23 +91,24 @@ weights_generic_kernel(const float *__restrict__ ref, float *__restrict__ w_out,
         const int y = (int)((vox / dm.X) % dm.Y), x = (int)(vox % dm.X);
         const int j = (ph + (s ? 1 : dm.P - 1)) % dm.P;
         const float *ri = ref + ph * V, *rj = ref + j * V;
+        float *w = w_out + ((size_t)ph * 2 + s) * nt * V + vox;   // w[k * V], k = 0 .. nt-1
         float Dm = INFINITY;
-        for (int tz = -dm.M; tz <= dm.M; ++tz)
-            for (int ty = -dm.M; ty <= dm.M; ++ty)
-                for (int tx = -dm.M; tx <= dm.M; ++tx)
-                    Dm = fminf(Dm, patch_distance(ri, rj, dm, z, y, x, tz, ty, tx));
-        float Zs = 0.f;
-        for (int tz = -dm.M; tz <= dm.M; ++tz)
-            for (int ty = -dm.M; ty <= dm.M; ++ty)
-                for (int tx = -dm.M; tx <= dm.M; ++tx)
-                    Zs += ex2((Dm - patch_distance(ri, rj, dm, z, y, x, tz, ty, tx)) * dm.c2);
-        const float inv = 1.0f / Zs;
         size_t k = 0;
         for (int tz = -dm.M; tz <= dm.M; ++tz)
             for (int ty = -dm.M; ty <= dm.M; ++ty)
-                for (int tx = -dm.M; tx <= dm.M; ++tx, ++k)
-                    w_out[(((size_t)ph * 2 + s) * nt + k) * V + vox] =
-                        ex2((Dm - patch_distance(ri, rj, dm, z, y, x, tz, ty, tx)) * dm.c2) * inv;
+                for (int tx = -dm.M; tx <= dm.M; ++tx, ++k) {
+                    const float D = patch_distance(ri, rj, dm, z, y, x, tz, ty, tx);
+                    w[k * V] = D;
+                    Dm = fminf(Dm, D);
+                }
+        float Zs = 0.f;
+        for (k = 0; k < nt; ++k) {
+            const float u = ex2((Dm - w[k * V]) * dm.c2);
+            w[k * V] = u;
+            Zs += u;
+        }
+        const float inv = 1.0f / Zs;
+        for (k = 0; k < nt; ++k) w[k * V] *= inv;
     }
 }
 

@@ -276,13 +276,9 @@ cudaError_t launch_pair5_t(const Dims &dm, const float *f, const float *g, float
 {
     using G = Pair5Geom<M, RZ, TX>;
     static_assert(NCTA * (G::BYTES + 1024) <= 228 * 1024, "NCTA tiles of the pair5 kernel do not fit in shared memory");
-    static bool configured = false;   // per template instance; the attribute is idempotent
-    cudaError_t e;
-    if (!configured) {
-        e = cudaFuncSetAttribute(tnlm_pair5_kernel<M, RZ, TX, NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<uint64_t> configured{0};   // per template instance: one bit per device
+    cudaError_t e = ensure_dynamic_smem(tnlm_pair5_kernel<M, RZ, TX, NCTA>, G::BYTES, configured);
+    if (e != cudaSuccess) return e;
     const int tiles_x = (dm.X + TX - 1) / TX;
     const int tiles_y = (dm.Y + kPair5RowsOut - 1) / kPair5RowsOut;
     const int tiles_z = (dm.z_end + RZ - 1) / RZ - dm.z_begin / RZ;   // tiles aligned to multiples of RZ

@@ -368,14 +368,9 @@ cudaError_t launch_tiled_t(const Dims &dm, const float *f, const float *g, float
 {
     using S = TiledSmem<M, XR, RZ>;
     using G = TiledGeom<M, XR>;
-    static bool configured = false;   // per template instance; the attribute is idempotent
-    cudaError_t e;
-    if (!configured) {
-        e = cudaFuncSetAttribute(tnlm_tiled_kernel<M, XR, RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)S::BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static std::atomic<uint64_t> configured{0};   // per template instance: one bit per device
+    cudaError_t e = ensure_dynamic_smem(tnlm_tiled_kernel<M, XR, RZ>, S::BYTES, configured);
+    if (e != cudaSuccess) return e;
     const int tiles_x = (dm.X + kTiledTX - 1) / kTiledTX;
     const int tiles_y = (dm.Y + kTiledRowsOut - 1) / kTiledRowsOut;
     const int tiles_z = (dm.z_end - dm.z_begin + RZ - 1) / RZ;

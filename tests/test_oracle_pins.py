@@ -420,3 +420,30 @@ def test_enhancement_denoises_config1(oracle):
     rmse0 = np.sqrt(((g - clean) ** 2).mean())
     rmse1 = np.sqrt(((f - clean) ** 2).mean())
     assert rmse1 < 0.6 * rmse0
+
+
+# --------------------------------------------------------------------------- finite dependence reach
+@pytest.mark.parametrize("d,M,K", [(1, 1, 2), (1, 2, 1), (2, 1, 1)])
+def test_trajectory_on_a_crop_equals_full_volume_inside_the_reach(oracle, d, M, K):
+    """Eq. 8 reads f and ref only within M+d voxels of x (PAPER.md:176 with the window of PAPER.md:223), so after
+    K sweeps a voxel depends on g within K(M+d) voxels.  An enhancement of a cropped stack therefore equals the
+    full-volume one, bit for bit, at every voxel further than K(M+d) from a cut face (faces that are faces of the
+    volume are not cuts: clamp-to-edge reads the same voxels, reading P4).  The GPU parity tests use this to check
+    whole 10-sweep trajectories at config 3 (tests/test_parity_trajectory_gpu.py); a wrong reach would show here as
+    a mismatch one voxel inside the claimed region, which is also asserted to exist."""
+    shape = (3, 15, 16, 17)
+    g = random_stack(shape, 77)
+    h, mu = np.float32(0.15), np.float32(0.5)
+    full = oracle.enhance(g, d, M, h, mu, K)
+    r = K * (M + d)
+    # corner crop: z, y, x faces at 0 are volume faces; the upper faces are cuts
+    zc, yc, xc = 15, 12, 13
+    crop = oracle.enhance(np.ascontiguousarray(g[:, :zc, :yc, :xc]), d, M, h, mu, K)
+    np.testing.assert_array_equal(crop[:, :, :yc - r, :xc - r], full[:, :zc, :yc - r, :xc - r])
+    # ... and the claim is sharp: within the reach of a cut face the crop does differ somewhere
+    assert np.any(crop[:, :, yc - r:, :] != full[:, :zc, yc - r:yc, :xc])
+    # interior crop: every face is a cut
+    a, b = 2, 14
+    crop = oracle.enhance(np.ascontiguousarray(g[:, :, a:b, a:b]), d, M, h, mu, K)
+    if b - a > 2 * r:
+        np.testing.assert_array_equal(crop[:, :, r:b - a - r, r:b - a - r], full[:, :, a + r:b - r, a + r:b - r])

@@ -189,15 +189,66 @@ def test_constant_stack_is_fixed_point_and_bounds(T):
         assert f.min().item() >= g.min().item() - 1e-6 and f.max().item() <= g.max().item() + 1e-6
 
 
-def test_weights_match_oracle(T, oracle):
-    shape = (3, 4, 6, 10)
+def _patch_distances(ref, d, M):
+    """D[p][s][k][z][y][x] of Eq. 3 in numpy fp64 (edge padding = reading P4; s = 0: phase p-1, s = 1: phase p+1;
+    k raster over (tz, ty, tx)): sets the scale of the fp32 error of each weight."""
+    P, Z, Y, X = ref.shape
+    R = M + d
+    pad = [np.pad(ref[i].astype(np.float64), R, mode="edge") for i in range(P)]
+    e = 2 * d + 1
+    out = np.empty((P, 2, (2 * M + 1) ** 3, Z, Y, X))
+    for i in range(P):
+        for s, j in enumerate(((i - 1) % P, (i + 1) % P)):
+            k = 0
+            for tz in range(-M, M + 1):
+                for ty in range(-M, M + 1):
+                    for tx in range(-M, M + 1):
+                        a = pad[i][M:M + Z + 2 * d, M:M + Y + 2 * d, M:M + X + 2 * d]
+                        b = pad[j][M + tz:M + tz + Z + 2 * d, M + ty:M + ty + Y + 2 * d, M + tx:M + tx + X + 2 * d]
+                        sq = (a - b) ** 2
+                        out[i, s, k] = np.lib.stride_tricks.sliding_window_view(sq, (e, e, e)).sum(axis=(-1, -2, -3))
+                        k += 1
+    return out
+
+
+@pytest.mark.parametrize("shape,d,M,h", [
+    ((3, 4, 6, 10), 1, 1, 0.2),
+    ((3, 5, 7, 9), 1, 2, 0.05),     # config 2/3's window and h: shifts of several hundred binades
+    ((3, 6, 7, 8), 2, 1, 0.1),      # 5^3 patch
+    ((2, 4, 9, 11), 1, 1, 0.02),    # tiny h: nearly one-hot weights, only the shifted form survives (reading P3)
+    ((3, 3, 5, 6), 0, 3, 0.3),      # single-voxel patch, 7^3 window larger than the volume
+])
+def test_weights_match_oracle(T, oracle, shape, d, M, h):
+    """tnlm_weights against the oracle's normalised weights of Eq. 3/9, every (p, s, k, x).
+
+    Tolerance from the arithmetic: the kernel forms D in fp32 (as the sweep kernels do).  A distance carries an
+    absolute error of at most ~8 ulp (sum of (2d+1)^3 squares, then parked as fp32), and w = 2^((Dmin - D) c2) / Z,
+    so |dw| <= w ln2 c2 * 8 * 2^-23 * (D + Dmin), plus 2e-6 for the exp2 approximation and the normalising sum.
+    D and Dmin come from numpy here (independent of both sides)."""
     ref = random_stack(shape, 21)
-    p = T.TnlmParams.make(shape, 1, 1, 0.2, 1.0)
-    want = oracle.weights(ref, 1, 1, np.float32(0.2))
+    p = T.TnlmParams.make(shape, d, M, h, 1.0)
+    want = oracle.weights(ref, d, M, np.float32(h))
     got = T.tnlm_weights(p, dev(ref)).cpu().numpy()
-    assert got.shape == want.shape and (got >= 0).all()
-    np.testing.assert_allclose(got.sum(axis=2), 1.0, atol=2e-6)
-    np.testing.assert_allclose(got, want, rtol=0, atol=2e-5)
+    n_t = (2 * M + 1) ** 3
+    assert got.shape == want.shape and (got >= 0).all() and np.isfinite(got).all()
+    np.testing.assert_allclose(got.sum(axis=2), 1.0, atol=n_t * 2.0 ** -23 + 1e-6)
+    c2 = 1.4426950408889634 / (2.0 * h * h)
+    D = _patch_distances(ref, d, M)
+    tol = want * np.log(2.0) * c2 * 8 * 2.0 ** -23 * (D + D.min(axis=2, keepdims=True)) + 2e-6
+    excess = np.abs(got - want) - tol
+    assert excess.max() <= 0, f"weight error exceeds the fp32 bound by {excess.max():.3e}"
+
+
+def test_weights_feed_the_sweep(T, oracle):
+    """The materialised weights reproduce the fused sweep: Eq. 8 evaluated with w_out (oracle's sweep_with_weights)
+    equals tnlm_jacobi_step on the same stack."""
+    shape = (3, 5, 8, 9)
+    f, g = random_stack(shape, 5), random_stack(shape, 6)
+    p = T.TnlmParams.make(shape, 1, 2, 0.15, 0.7)
+    w = T.tnlm_weights(p, dev(f)).cpu().numpy().astype(np.float64)
+    via_w = oracle.sweep_with_weights_f64(f, g, w, 2, 0.7)
+    got = T.tnlm_jacobi_step(p, dev(f), dev(g)).cpu().numpy()
+    assert_parity(got, via_w, 1.0, "sweep from materialised weights")
 
 
 # ------------------------------------------------------------------ loop / ABI semantics on the device
@@ -384,3 +435,34 @@ def test_fuzz_packed_kernels_against_generic(T):
         T.tnlm_jacobi_step_slab(p, f, g, za, zb, f_out=out, variant=T.VARIANT_PAIRED)
         assert torch.equal(out[:, za:zb], got[:, za:zb]), f"case {case}: slab [{za},{zb}) differs from the full sweep"
         assert (out[:, :za] == -3.0).all() and (out[:, zb:] == -3.0).all(), f"case {case}: slab wrote outside [{za},{zb})"
+
+
+# ------------------------------------------------------------------ memory safety without compute-sanitizer
+@pytest.mark.parametrize("shape,d,M", [((3, 7, 31, 33), 1, 2), ((2, 9, 30, 17), 1, 1), ((2, 5, 29, 35), 1, 3), ((2, 6, 33, 19), 1, 4),
+                                       ((3, 6, 29, 18), 2, 1), ((2, 7, 28, 34), 2, 2), ((2, 5, 31, 21), 2, 4), ((2, 3, 5, 7), 3, 5)])
+def test_guard_regions_stay_untouched(T, shape, d, M):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are looked for directly: f_out and the
+    workspace sit inside larger allocations whose guard regions (4 KB either side) hold a canary pattern, and every
+    kernel variant, full sweeps and slabs, must leave the canaries and the planes outside a slab intact."""
+    import torch
+    n = int(np.prod(shape))
+    G = 1024                                                       # guard floats
+    f, g = dev(random_stack(shape, 51)), dev(random_stack(shape, 52))
+    p = T.TnlmParams.make(shape, d, M, 0.2, 0.5)
+    wsb = T.workspace_bytes(p)
+    for v in variants(T, p):
+        buf = torch.full((n + 2 * G,), -123.25, device="cuda")
+        wbuf = torch.full((wsb + 8192,), 0x5A, dtype=torch.uint8, device="cuda")
+        out = buf[G:G + n].view(shape)
+        ws = wbuf[4096:4096 + wsb]
+        assert out.data_ptr() % 16 == 0 and ws.data_ptr() % 16 == 0
+        T.tnlm_jacobi_step(p, f, g, f_out=out, ws=ws, variant=v)
+        T.tnlm_enhance(p, g, 2, f_out=out, ws=ws, variant=v)
+        za, zb = 1, max(1, shape[1] - 1)
+        out.fill_(-7.5)
+        T.tnlm_jacobi_step_slab(p, f, g, za, zb, f_out=out, ws=ws, variant=v)
+        torch.cuda.synchronize()
+        assert (buf[:G] == -123.25).all() and (buf[G + n:] == -123.25).all(), f"variant {v}: wrote outside f_out"
+        assert (wbuf[:4096] == 0x5A).all() and (wbuf[4096 + wsb:] == 0x5A).all(), f"variant {v}: wrote outside the workspace"
+        assert (out[:, :za] == -7.5).all() and (out[:, zb:] == -7.5).all(), f"variant {v}: slab sweep wrote outside its planes"
+        assert out[:, za:zb].isfinite().all()
