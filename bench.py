@@ -49,6 +49,9 @@ def parse_args():
                     help="config1..config4: one enhancement per step; config5: the (patch, window) sweep of "
                          "BASELINE.json configs[4], one step = the eight enhancements, per-point figures in 'points'")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant: 0 auto, 1 generic, 2 tiled, 3 paired")
+    ap.add_argument("--ref", default="same", choices=["same", "separate"],
+                    help="separate: every sweep takes its weights from a second stack (tnlm_jacobi_step(ref=...), "
+                         "the TNLM-R form of the call, PAPER.md:198) instead of from the iterate; no e2e leg")
     ap.add_argument("--metrics", action="store_true",
                     help="also evaluate the paper's SRR (Eq. 10) and CNR on the enhanced stack and time the TV kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -324,11 +327,23 @@ def main():
     stack_mb = g.numel() * 4 / 1e6
     flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev) if 3 * stack_mb <= 126 else None
 
+    sep = args.ref == "separate"
+    if sep:   # weights from a lightly smoothed copy of the stack, as an outer TNLM-R iteration would pass
+        ref_stack = (0.5 * g + 0.25 * torch.roll(g, 1, 3) + 0.25 * torch.roll(g, -1, 3)).contiguous()
+        f_tmp = torch.empty_like(g)
+        args.no_e2e = True
+
     def step(record=None):
         for k, (c, p) in enumerate(points):
             if record is not None:
                 record[k][0].record(stream)
-            T.tnlm_enhance(p, g, c.n_iter, f_out=f_out, ws=ws, stream=stream, variant=args.variant)
+            if sep:
+                src, dst = g, (f_out if c.n_iter % 2 == 1 else f_tmp)
+                for _ in range(c.n_iter):
+                    T.tnlm_jacobi_step(p, src, g, ref=ref_stack, f_out=dst, ws=ws, stream=stream, variant=args.variant)
+                    src, dst = dst, (f_tmp if dst is f_out else f_out)
+            else:
+                T.tnlm_enhance(p, g, c.n_iter, f_out=f_out, ws=ws, stream=stream, variant=args.variant)
             if record is not None:
                 record[k][1].record(stream)
         if flush is not None:
@@ -439,8 +454,12 @@ def main():
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": workload_config(cfg, info.world, sweep_mode), "clocks": clocks, "e2e": e2e,
         "gpu_launches": args.steps * launches_per_step, "roofline": roofline, "cpu_baseline": cpu_baseline,
-        "impl": "tnlm", "kernel": roofline["kernel"], "variant": args.variant,
+        "impl": "tnlm", "kernel": roofline["kernel"], "variant": args.variant, "ref": args.ref,
     }
+    if sep:
+        line["config"]["workload"] += "; weights of every sweep from a SEPARATE stack (tnlm_jacobi_step(ref=...))"
+        line["kernel"] = roofline["kernel"] = roofline["kernel"] + " (separate ref: candidate tile)"
+        roofline["traffic"] = None
     if sweep_mode:
         line["points"] = point_lines
     if quality:

@@ -62,8 +62,9 @@ typedef enum {
 /* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M):
  *   GENERIC  any d <= 3, M <= 6, any ref: one thread per voxel, loops as the definition
  *   TILED    d = 1, 1 <= M <= 4, ref == f: scalar FP32 tiles (first optimised kernel, kept for cross-checks)
- *   PAIRED   d = 1 or 2, 1 <= M <= 4, ref == f: row-pair packed FP32 (FADD2 / FFMA2) -- what AUTO selects there
- * With AUTO a separate ref (ref != f) takes GENERIC. */
+ *   PAIRED   d = 1 or 2, 1 <= M <= 4, any ref: row-pair packed FP32 (FADD2 / FFMA2) -- what AUTO selects there
+ *            (with ref != f the kernel keeps a second neighbour tile for the candidate values: smaller tiles, slower)
+ * A separate ref with TILED is refused (TNLM_ERR_UNSUPPORTED). */
 enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2, TNLM_VARIANT_PAIRED = 3 };
 
 /*

@@ -161,7 +161,7 @@ int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const fl
     int v = pick_variant(p, variant);
     if (v < 0) return TNLM_ERR_UNSUPPORTED;
     if (!ref) ref = f;
-    if ((v == TNLM_VARIANT_TILED || v == TNLM_VARIANT_PAIRED) && ref != f) {   // these cover TNLM-E (ref = f) only
+    if (v == TNLM_VARIANT_TILED && ref != f) {   // the scalar tiled kernel covers TNLM-E (ref = f) only
         if (variant != TNLM_VARIANT_AUTO) return TNLM_ERR_UNSUPPORTED;
         v = TNLM_VARIANT_GENERIC;
     }

@@ -27,6 +27,9 @@
 //       a4  Z += u, N += u * f_j(x+t)                                         FADD2 + FFMA2
 //   epilogue    = NLM of the first direction is parked in f_out (same thread reads it back), then
 //                 a5: f_out = mu/(2+mu) g + (NLM- + NLM+)/(2+mu)
+// SEP = true (ref != f: weights from another stack than the one that is averaged): a third tile F holds
+// f_j in the layout of B (both copies) for the planes that carry candidates; the candidate window of a pass is read
+// from F instead of being the centre of the B window of the previous plane.
 // Reference exponent (reading P3: weights relative to the best candidate).  Every output keeps a
 // reference exponent b; a pass sums its W terms ex2(b - c2*D) optimistically.  If the partial
 // normaliser stays below 2^100 (no candidate ~2^100 times better than the reference) it is added as
@@ -57,7 +60,7 @@ __device__ __forceinline__ float2 add2(const float2 a, const float2 b) { return 
 __device__ __forceinline__ float2 mul2(const float2 a, const float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 fma2(const float2 a, const float2 b, const float2 c) { return __ffma2_rn(a, b, c); }
 
-template <int M, int RZ, int TX> struct PairGeom {
+template <int M, int RZ, int TX, bool SEP = false> struct PairGeom {
     using C = Chunks<M>;
     static constexpr int E = 2 * M + 1;
     static constexpr int NRUN = TX / 2;             // x-runs of 2 voxels
@@ -71,8 +74,9 @@ template <int M, int RZ, int TX> struct PairGeom {
     static constexpr int NPA = 16, NPE = 16 + M, NPO = 15 + M;     // row pairs per plane
     static constexpr int NPB = NPE + NPO;                          // a B plane = its BE pairs, then its BO pairs
     static constexpr int NAP = RZ + 2, NBP = RZ + 2 + 2 * M;       // planes
-    static constexpr int A_F2 = NAP * NPA * PA2, B_F2 = NBP * NPB * PB2;
-    static constexpr size_t BYTES = (size_t)(A_F2 + B_F2) * sizeof(float2);
+    static constexpr int NFP = SEP ? RZ + 2 * M : 0;               // planes of the candidate tile F: B planes 1 .. NBP-2
+    static constexpr int A_F2 = NAP * NPA * PA2, B_F2 = NBP * NPB * PB2, F_F2 = NFP * NPB * PB2;
+    static constexpr size_t BYTES = (size_t)(A_F2 + B_F2 + F_F2) * sizeof(float2);
 };
 
 struct AccPair { float2 z[2], n[2], b[2]; };   // [x of the run]; .x = row 2l, .y = row 2l+1
@@ -107,9 +111,11 @@ __device__ __forceinline__ void load_pairs(const float2 *__restrict__ p, float2 
 //   c2*Dmin of the chunk (with headroom) if that beats its reference by more than 2^97, branch-free, and the
 //   terms are evaluated once.  Used for the first chunk (reference = +inf) and to re-do a chunk that reported failures.
 // Both forms execute the same shuffles, so a warp may run them with different masks per lane.
-template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE>
+//   fRow (SEP only): &F?[plane tz][pair l + ty/2][x0 + q0], F plane k <-> B plane k + 1
+template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE, bool SEP = false>
 __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
-                                              const float c2, AccPair (&acc)[RZ], const unsigned mask)
+                                              const float2 *__restrict__ fRow, const float c2, AccPair (&acc)[RZ],
+                                              const unsigned mask)
 {
     constexpr int NVB = (W + 4) / 2;
     const float2 nc2 = make_float2(-c2, -c2);
@@ -133,6 +139,7 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
         }
         if (p >= 2) {
             AccPair &ac = acc[p - 2];
+            if (SEP) load_pairs<NVB>(fRow + (p - 2) * B_PLANE, bprev);   // candidates f_j(x+t) of the centre plane
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 float2 D[W];
@@ -199,8 +206,10 @@ __device__ __forceinline__ unsigned pair_pass(const float2 *__restrict__ aRow, c
                 ring0[q][i] = ring1[q][i];
                 ring1[q][i] = X[q][i];
             }
+        if (!SEP) {
 #pragma unroll
-        for (int k = 0; k < 2 * NVB; ++k) bprev[k] = b[k];
+            for (int k = 0; k < 2 * NVB; ++k) bprev[k] = b[k];
+        }
     }
     return fail;
 }
@@ -258,18 +267,20 @@ __device__ __forceinline__ void stage_pairs(float *__restrict__ dstE, float *__r
     }
 }
 
-template <int M, int RZ, int TX, int NCTA>
-__global__ void __launch_bounds__(PairGeom<M, RZ, TX>::NT, NCTA)
-tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float *f_out, const Dims dm,
-                 const int tiles_x, const int tiles_y, const int tiles_z)
+template <int M, int RZ, int TX, int NCTA, bool SEP = false>
+__global__ void __launch_bounds__(PairGeom<M, RZ, TX, SEP>::NT, NCTA)
+tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, const float *__restrict__ ref, float *f_out,
+                 const Dims dm, const int tiles_x, const int tiles_y, const int tiles_z)
 {
-    using G = PairGeom<M, RZ, TX>;
+    using G = PairGeom<M, RZ, TX, SEP>;
     using C = Chunks<M>;
     constexpr int AP = G::NPA * G::PA2, BP = G::NPB * G::PB2;   // plane strides (float2)
     extern __shared__ __align__(16) float smem[];
     float2 *sA = reinterpret_cast<float2 *>(smem);
     float2 *sBE = sA + G::A_F2;
     float2 *sBO = sBE + G::NPE * G::PB2;   // odd pairs of plane 0
+    float2 *sFE = sBE + G::B_F2;           // SEP: candidate tile, same plane layout as B
+    float2 *sFO = sFE + G::NPE * G::PB2;
 
     int t = blockIdx.x;
     const int bx = t % tiles_x; t /= tiles_x;
@@ -286,7 +297,7 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
 
     // -ref_i tile (halo 1): rows <-> y = Y0-1+r, cols <-> x = X0-1+c, planes <-> z = Z0-1+pz
     stage_pairs<G::PA2, 32, G::ACOLS, G::NAP, G::NPA, 0, true, G::NT>(
-        reinterpret_cast<float *>(sA), nullptr, f + (size_t)ph * V, Z0 - 1, Y0 - 1, X0 - 1, dm, tid);
+        reinterpret_cast<float *>(sA), nullptr, ref + (size_t)ph * V, Z0 - 1, Y0 - 1, X0 - 1, dm, tid);
 
     const size_t zstride = (size_t)dm.Y * dm.X;
     const bool vec_ok = (dm.X % 2) == 0;
@@ -296,10 +307,14 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
     for (int s = 0; s < 2; ++s) {
         const int j = (ph + (s ? 1 : dm.P - 1)) % dm.P;
         __syncthreads();   // everyone is done with the previous B tiles
-        // f_j tiles (halo 1+M): rows <-> y = Y0-1-M+r, cols <-> x = X0-1-M+c, planes <-> z = Z0-1-M+pz
+        // ref_j tiles (halo 1+M): rows <-> y = Y0-1-M+r, cols <-> x = X0-1-M+c, planes <-> z = Z0-1-M+pz
         stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NBP, G::NPE, G::NPO, false, G::NT>(
-            reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), f + (size_t)j * V, Z0 - 1 - M, Y0 - 1 - M,
+            reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), ref + (size_t)j * V, Z0 - 1 - M, Y0 - 1 - M,
             X0 - 1 - M, dm, tid);
+        if constexpr (SEP)   // f_j, same rows and columns, planes <-> z = Z0-M+pz
+            stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NFP, G::NPE, G::NPO, false, G::NT>(
+                reinterpret_cast<float *>(sFE), reinterpret_cast<float *>(sFO), f + (size_t)j * V, Z0 - M, Y0 - 1 - M,
+                X0 - 1 - M, dm, tid);
         __syncthreads();
 
         AccPair acc[RZ];
@@ -316,9 +331,10 @@ tnlm_pair_kernel(const float *__restrict__ f, const float *__restrict__ g, float
         // warp re-does the chunk in the careful form (each lane with its own mask of failed row pairs)
         auto run_chunk = [&](auto wtag, const float2 *bRow, const bool first) {
             constexpr int W = decltype(wtag)::value;
+            const float2 *fRow = bRow + (sFE - sBE);   // same (plane, pair, column) of the candidate tile
             unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
-            if (!first) fail = pair_pass<RZ, W, false, AP, BP>(aRow, bRow, dm.c2, acc, 0u);
-            if (__any_sync(0xffffffffu, fail != 0u)) pair_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail);
+            if (!first) fail = pair_pass<RZ, W, false, AP, BP, SEP>(aRow, bRow, fRow, dm.c2, acc, 0u);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair_pass<RZ, W, true, AP, BP, SEP>(aRow, bRow, fRow, dm.c2, acc, fail);
         };
 #pragma unroll 1
         for (int k = 0; k < G::E * G::E; ++k) {
@@ -419,34 +435,42 @@ inline const char *pair_name(const tnlm_params &p)
     }
 }
 
-template <int M, int RZ, int TX, int NCTA>
-cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, float *f_out, cudaStream_t st)
+template <int M, int RZ, int TX, int NCTA, bool SEP = false>
+cudaError_t launch_pair_t(const Dims &dm, const float *f, const float *g, const float *ref, float *f_out, cudaStream_t st)
 {
-    using G = PairGeom<M, RZ, TX>;
+    using G = PairGeom<M, RZ, TX, SEP>;
     static_assert(NCTA * (G::BYTES + 1024) <= 228 * 1024, "NCTA tiles of the pair kernel do not fit in shared memory");
     static std::atomic<uint64_t> configured{0};   // per template instance: one bit per device
-    cudaError_t e = ensure_dynamic_smem(tnlm_pair_kernel<M, RZ, TX, NCTA>, G::BYTES, configured);
+    cudaError_t e = ensure_dynamic_smem(tnlm_pair_kernel<M, RZ, TX, NCTA, SEP>, G::BYTES, configured);
     if (e != cudaSuccess) return e;
     const int tiles_x = (dm.X + TX - 1) / TX;
     const int tiles_y = (dm.Y + kPairRowsOut - 1) / kPairRowsOut;
     const int tiles_z = (dm.z_end + RZ - 1) / RZ - dm.z_begin / RZ;   // tiles aligned to multiples of RZ
     const long long blocks = (long long)tiles_x * tiles_y * tiles_z * dm.P;
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
-    tnlm_pair_kernel<M, RZ, TX, NCTA><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
+    tnlm_pair_kernel<M, RZ, TX, NCTA, SEP><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, ref, f_out, dm, tiles_x, tiles_y, tiles_z);
     return cudaGetLastError();
 }
 
-// ref must be f (TNLM-E); the caller falls back to the generic kernel otherwise.
+// <M, RZ, TX, CTAs per SM>: the shapes that measured best on the thorax phantoms.  With a
+// separate ref stack the candidate tile F needs room of its own: shallower or narrower tiles, fewer CTAs per SM.
 inline cudaError_t launch_pair(const tnlm_params &p, const Dims &dm, const float *f, const float *g, const float *ref,
                                float *f_out, cudaStream_t st)
 {
-    if (ref != f) return cudaErrorNotSupported;
-    // <M, RZ, TX, CTAs per SM>: the shapes that measured best on the thorax phantoms
+    if (ref == f) {
+        switch (p.search_radius) {
+            case 1: return launch_pair_t<1, 4, 16, 3>(dm, f, g, f, f_out, st);
+            case 2: return launch_pair_t<2, 4, 16, 3>(dm, f, g, f, f_out, st);
+            case 3: return launch_pair_t<3, 6, 32, 1>(dm, f, g, f, f_out, st);
+            case 4: return launch_pair_t<4, 4, 32, 1>(dm, f, g, f, f_out, st);
+            default: return cudaErrorNotSupported;
+        }
+    }
     switch (p.search_radius) {
-        case 1: return launch_pair_t<1, 4, 16, 3>(dm, f, g, f_out, st);
-        case 2: return launch_pair_t<2, 4, 16, 3>(dm, f, g, f_out, st);
-        case 3: return launch_pair_t<3, 6, 32, 1>(dm, f, g, f_out, st);
-        case 4: return launch_pair_t<4, 4, 32, 1>(dm, f, g, f_out, st);
+        case 1: return launch_pair_t<1, 4, 16, 2, true>(dm, f, g, ref, f_out, st);
+        case 2: return launch_pair_t<2, 4, 32, 1, true>(dm, f, g, ref, f_out, st);
+        case 3: return launch_pair_t<3, 2, 24, 1, true>(dm, f, g, ref, f_out, st);
+        case 4: return launch_pair_t<4, 2, 16, 1, true>(dm, f, g, ref, f_out, st);
         default: return cudaErrorNotSupported;
     }
 }

@@ -19,7 +19,7 @@ constexpr int kPair5RowsOut = 28;
 // chunk c of the 2M+1 x-offsets: starts at q0 = 2c; width 2, the last chunk (c = M-1) 3
 __host__ __device__ constexpr int chunk5_w(int M, int c) { return c == M - 1 ? 3 : 2; }
 
-template <int M, int RZ, int TX> struct Pair5Geom {
+template <int M, int RZ, int TX, bool SEP = false> struct Pair5Geom {
     static constexpr int E = 2 * M + 1;
     static constexpr int NRUN = TX / 2, NT = NRUN * 16;
     static constexpr int ACOLS = TX + 4, BCOLS = TX + 2 * M + 4;      // staged columns
@@ -29,17 +29,20 @@ template <int M, int RZ, int TX> struct Pair5Geom {
     static constexpr int PB2 = pitch2(cmax(BCOLS, BREAD));
     static constexpr int NPA = 16, NPE = 16 + M, NPO = 15 + M, NPB = NPE + NPO;
     static constexpr int NAP = RZ + 4, NBP = RZ + 4 + 2 * M;
-    static constexpr int A_F2 = NAP * NPA * PA2, B_F2 = NBP * NPB * PB2;
-    static constexpr size_t BYTES = (size_t)(A_F2 + B_F2) * sizeof(float2);
+    static constexpr int NFP = SEP ? RZ + 2 * M : 0;                  // candidate tile F (ref != f): B planes 2 .. NBP-3
+    static constexpr int A_F2 = NAP * NPA * PA2, B_F2 = NBP * NPB * PB2, F_F2 = NFP * NPB * PB2;
+    static constexpr size_t BYTES = (size_t)(A_F2 + B_F2 + F_F2) * sizeof(float2);
 };
 
 // One pass of the 5^3-patch kernel: W consecutive x-offsets at fixed (ty, tz), marching the RZ+4 planes.
 //   aRow: &A2[plane 0][pair l][x0]                 element k <-> x = X0 + x0 - 2 + k   (negated values)
 //   bRow: &B?[plane tz][pair l + ty/2][x0 + q0]    element k + q pairs with a[k] for the q-th offset of the chunk
-// CAREFUL as in pair_pass (tnlm_pair.cuh).
-template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE>
+//   fRow (SEP only): &F?[plane tz][pair l + ty/2][x0 + q0], F plane k <-> B plane k + 2
+// CAREFUL and SEP as in pair_pass (tnlm_pair.cuh).
+template <int RZ, int W, bool CAREFUL, int A_PLANE, int B_PLANE, bool SEP = false>
 __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, const float2 *__restrict__ bRow,
-                                               const float c2, AccPair (&acc)[RZ], const unsigned mask)
+                                               const float2 *__restrict__ fRow, const float c2, AccPair (&acc)[RZ],
+                                               const unsigned mask)
 {
     constexpr int NVB = (W + 6) / 2;   // 6 + W - 1 positions
     const float2 nc2 = make_float2(-c2, -c2);
@@ -66,6 +69,12 @@ __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, 
         }
         if (p >= 4) {
             AccPair &ac = acc[p - 4];
+            if (SEP) {   // candidates f_j(x+t) of the centre plane: window elements 2 .. W+2
+                float2 fw[2 * NVB];
+                load_pairs<NVB>(fRow + (p - 4) * B_PLANE, fw);
+#pragma unroll
+                for (int k = 0; k < W + 1; ++k) cand2[k] = fw[k + 2];
+            }
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 float2 D[W];
@@ -130,26 +139,30 @@ __device__ __forceinline__ unsigned pair5_pass(const float2 *__restrict__ aRow, 
                 ring[3][q][i] = X[q][i];
             }
         // output x-index i, offset q reads the candidate at window element i + 2 + q
+        if (!SEP) {
 #pragma unroll
-        for (int k = 0; k < W + 1; ++k) {
-            cand2[k] = cand1[k];
-            cand1[k] = b[k + 2];
+            for (int k = 0; k < W + 1; ++k) {
+                cand2[k] = cand1[k];
+                cand1[k] = b[k + 2];
+            }
         }
     }
     return fail;
 }
 
-template <int M, int RZ, int TX, int NCTA>
-__global__ void __launch_bounds__(Pair5Geom<M, RZ, TX>::NT, NCTA)
-tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, float *f_out, const Dims dm,
-                  const int tiles_x, const int tiles_y, const int tiles_z)
+template <int M, int RZ, int TX, int NCTA, bool SEP = false>
+__global__ void __launch_bounds__(Pair5Geom<M, RZ, TX, SEP>::NT, NCTA)
+tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, const float *__restrict__ ref, float *f_out,
+                  const Dims dm, const int tiles_x, const int tiles_y, const int tiles_z)
 {
-    using G = Pair5Geom<M, RZ, TX>;
+    using G = Pair5Geom<M, RZ, TX, SEP>;
     constexpr int AP = G::NPA * G::PA2, BP = G::NPB * G::PB2;   // plane strides (float2)
     extern __shared__ __align__(16) float smem[];
     float2 *sA = reinterpret_cast<float2 *>(smem);
     float2 *sBE = sA + G::A_F2;
     float2 *sBO = sBE + G::NPE * G::PB2;   // odd pairs of plane 0
+    float2 *sFE = sBE + G::B_F2;           // SEP: candidate tile, same plane layout as B
+    float2 *sFO = sFE + G::NPE * G::PB2;
 
     int t = blockIdx.x;
     const int bx = t % tiles_x; t /= tiles_x;
@@ -165,7 +178,7 @@ tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, floa
 
     // -ref_i tile (halo 2): rows <-> y = Y0-2+r, cols <-> x = X0-2+c, planes <-> z = Z0-2+pz
     stage_pairs<G::PA2, 32, G::ACOLS, G::NAP, G::NPA, 0, true, G::NT>(
-        reinterpret_cast<float *>(sA), nullptr, f + (size_t)ph * V, Z0 - 2, Y0 - 2, X0 - 2, dm, tid);
+        reinterpret_cast<float *>(sA), nullptr, ref + (size_t)ph * V, Z0 - 2, Y0 - 2, X0 - 2, dm, tid);
 
     const size_t zstride = (size_t)dm.Y * dm.X;
     const bool vec_ok = (dm.X % 2) == 0;
@@ -175,10 +188,14 @@ tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, floa
     for (int s = 0; s < 2; ++s) {
         const int j = (ph + (s ? 1 : dm.P - 1)) % dm.P;
         __syncthreads();   // everyone is done with the previous B tiles
-        // f_j tiles (halo 2+M): rows <-> y = Y0-2-M+r, cols <-> x = X0-2-M+c, planes <-> z = Z0-2-M+pz
+        // ref_j tiles (halo 2+M): rows <-> y = Y0-2-M+r, cols <-> x = X0-2-M+c, planes <-> z = Z0-2-M+pz
         stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NBP, G::NPE, G::NPO, false, G::NT>(
-            reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), f + (size_t)j * V, Z0 - 2 - M, Y0 - 2 - M,
+            reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO), ref + (size_t)j * V, Z0 - 2 - M, Y0 - 2 - M,
             X0 - 2 - M, dm, tid);
+        if constexpr (SEP)   // f_j, same rows and columns, planes <-> z = Z0-M+pz
+            stage_pairs<G::PB2, 32 + 2 * M, G::BCOLS, G::NFP, G::NPE, G::NPO, false, G::NT>(
+                reinterpret_cast<float *>(sFE), reinterpret_cast<float *>(sFO), f + (size_t)j * V, Z0 - M, Y0 - 2 - M,
+                X0 - 2 - M, dm, tid);
         __syncthreads();
 
         AccPair acc[RZ];
@@ -193,9 +210,10 @@ tnlm_pair5_kernel(const float *__restrict__ f, const float *__restrict__ g, floa
         const float2 *aRow = sA + l * G::PA2 + x0;
         auto run_chunk = [&](auto wtag, const float2 *bRow, const bool first) {
             constexpr int W = decltype(wtag)::value;
+            const float2 *fRow = bRow + (sFE - sBE);   // same (plane, pair, column) of the candidate tile
             unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
-            if (!first) fail = pair5_pass<RZ, W, false, AP, BP>(aRow, bRow, dm.c2, acc, 0u);
-            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP>(aRow, bRow, dm.c2, acc, fail);
+            if (!first) fail = pair5_pass<RZ, W, false, AP, BP, SEP>(aRow, bRow, fRow, dm.c2, acc, 0u);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass<RZ, W, true, AP, BP, SEP>(aRow, bRow, fRow, dm.c2, acc, fail);
         };
 #pragma unroll 1
         for (int k = 0; k < G::E * G::E; ++k) {
@@ -271,33 +289,41 @@ inline const char *pair5_name(const tnlm_params &p)
     }
 }
 
-template <int M, int RZ, int TX, int NCTA>
-cudaError_t launch_pair5_t(const Dims &dm, const float *f, const float *g, float *f_out, cudaStream_t st)
+template <int M, int RZ, int TX, int NCTA, bool SEP = false>
+cudaError_t launch_pair5_t(const Dims &dm, const float *f, const float *g, const float *ref, float *f_out, cudaStream_t st)
 {
-    using G = Pair5Geom<M, RZ, TX>;
+    using G = Pair5Geom<M, RZ, TX, SEP>;
     static_assert(NCTA * (G::BYTES + 1024) <= 228 * 1024, "NCTA tiles of the pair5 kernel do not fit in shared memory");
     static std::atomic<uint64_t> configured{0};   // per template instance: one bit per device
-    cudaError_t e = ensure_dynamic_smem(tnlm_pair5_kernel<M, RZ, TX, NCTA>, G::BYTES, configured);
+    cudaError_t e = ensure_dynamic_smem(tnlm_pair5_kernel<M, RZ, TX, NCTA, SEP>, G::BYTES, configured);
     if (e != cudaSuccess) return e;
     const int tiles_x = (dm.X + TX - 1) / TX;
     const int tiles_y = (dm.Y + kPair5RowsOut - 1) / kPair5RowsOut;
     const int tiles_z = (dm.z_end + RZ - 1) / RZ - dm.z_begin / RZ;   // tiles aligned to multiples of RZ
     const long long blocks = (long long)tiles_x * tiles_y * tiles_z * dm.P;
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
-    tnlm_pair5_kernel<M, RZ, TX, NCTA><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
+    tnlm_pair5_kernel<M, RZ, TX, NCTA, SEP><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, ref, f_out, dm, tiles_x, tiles_y, tiles_z);
     return cudaGetLastError();
 }
 
-// ref must be f (TNLM-E); the caller falls back to the generic kernel otherwise.
+// With a separate ref stack the candidate tile F needs room of its own: shallower or narrower tiles (see launch_pair).
 inline cudaError_t launch_pair5(const tnlm_params &p, const Dims &dm, const float *f, const float *g, const float *ref,
                                 float *f_out, cudaStream_t st)
 {
-    if (ref != f) return cudaErrorNotSupported;
+    if (ref == f) {
+        switch (p.search_radius) {
+            case 1: return launch_pair5_t<1, 6, 16, 2>(dm, f, g, f, f_out, st);
+            case 2: return launch_pair5_t<2, 4, 16, 2>(dm, f, g, f, f_out, st);
+            case 3: return launch_pair5_t<3, 4, 32, 1>(dm, f, g, f, f_out, st);
+            case 4: return launch_pair5_t<4, 2, 32, 1>(dm, f, g, f, f_out, st);
+            default: return cudaErrorNotSupported;
+        }
+    }
     switch (p.search_radius) {
-        case 1: return launch_pair5_t<1, 6, 16, 2>(dm, f, g, f_out, st);
-        case 2: return launch_pair5_t<2, 4, 16, 2>(dm, f, g, f_out, st);
-        case 3: return launch_pair5_t<3, 4, 32, 1>(dm, f, g, f_out, st);
-        case 4: return launch_pair5_t<4, 2, 32, 1>(dm, f, g, f_out, st);
+        case 1: return launch_pair5_t<1, 4, 32, 1, true>(dm, f, g, ref, f_out, st);
+        case 2: return launch_pair5_t<2, 2, 32, 1, true>(dm, f, g, ref, f_out, st);
+        case 3: return launch_pair5_t<3, 2, 16, 1, true>(dm, f, g, ref, f_out, st);
+        case 4: return launch_pair5_t<4, 2, 8, 1, true>(dm, f, g, ref, f_out, st);
         default: return cudaErrorNotSupported;
     }
 }

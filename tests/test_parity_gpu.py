@@ -160,20 +160,40 @@ def test_ragged_tiles_one_sweep(T, oracle, shape):
             assert_parity(got, want, 1.0, f"ragged {shape} M={M} variant {v}")
 
 
-def test_separate_ref_stack(T, oracle):
-    """TNLM-R usage: weights from ref = g^(k), averages of f."""
-    shape = (3, 9, 20, 41)
+@pytest.mark.parametrize("d,M,shape", [(1, 1, (3, 9, 33, 41)), (1, 2, (3, 9, 35, 41)), (1, 3, (3, 7, 33, 29)), (1, 4, (2, 6, 31, 21)),
+                                       (2, 1, (3, 9, 31, 37)), (2, 2, (3, 7, 30, 35)), (2, 3, (2, 6, 29, 19)), (2, 4, (2, 5, 29, 13))])
+def test_separate_ref_stack(T, oracle, d, M, shape):
+    """ref != f (weights from one stack, averages of another): every kernel variant that takes a
+    separate ref, the packed kernels included (they hold f_j in a candidate tile of its own), against the oracle."""
     f, g, ref = random_stack(shape, 1), random_stack(shape, 2), random_stack(shape, 3)
-    p = T.TnlmParams.make(shape, 1, 2, 0.3, 0.5)
-    want = oracle.jacobi_step(f, g, 1, 2, np.float32(0.3), np.float32(0.5), ref=ref)
-    # the tiled kernel covers ref = f only: AUTO falls back to the generic kernel, an explicit request is refused
-    for v in (T.VARIANT_GENERIC, T.VARIANT_AUTO):
+    h = 0.3 if d == 1 else 0.45
+    p = T.TnlmParams.make(shape, d, M, h, 0.5)
+    want = oracle.jacobi_step(f, g, d, M, np.float32(h), np.float32(0.5), ref=ref)
+    for v in (T.VARIANT_GENERIC, T.VARIANT_PAIRED, T.VARIANT_AUTO):
         got = T.tnlm_jacobi_step(p, dev(f), dev(g), ref=dev(ref), variant=v).cpu().numpy()
-        assert_parity(got, want, 1.0, f"separate ref variant {v}")
-    if T.VARIANT_TILED in variants(T, p):
+        assert_parity(got, want, 1.0, f"separate ref d={d} M={M} variant {v}")
+    if T.VARIANT_TILED in variants(T, p):      # the scalar tiled kernel covers ref = f only: an explicit request is refused
         with pytest.raises(T.TnlmError) as e:
             T.tnlm_jacobi_step(p, dev(f), dev(g), ref=dev(ref), variant=T.VARIANT_TILED)
         assert e.value.code == -4
+
+
+def test_separate_ref_thorax_moving_edges(T, oracle):
+    """Separate ref on structured data: weights from a lightly smoothed copy (what a TNLM-R outer iteration would
+    pass), values from the noisy stack; slabs of the packed kernel tile the sweep bit for bit there too."""
+    import torch
+    cfg = CONFIGS["config2"].scaled(nz=13, ny=47, nx=50, n_phase=4, tumour_radius=3, si_amplitude=3)
+    g = make_stack(cfg)
+    ref = (0.5 * g + 0.25 * np.roll(g, 1, axis=3) + 0.25 * np.roll(g, -1, axis=3)).astype(np.float32)
+    for d, M, h in [(1, 2, 0.05), (2, 1, 0.08)]:
+        p = T.TnlmParams.make(cfg.shape, d, M, h, cfg.mu)
+        want = oracle.jacobi_step(g, g, d, M, np.float32(h), np.float32(cfg.mu), ref=ref)
+        got = T.tnlm_jacobi_step(p, dev(g), dev(g), ref=dev(ref), variant=T.VARIANT_PAIRED)
+        assert_parity(got.cpu().numpy(), want, dynamic_range(g), f"separate ref thorax d={d} M={M}")
+        out = torch.full_like(got, -5.0)
+        for (a, b) in [(0, 3), (3, 4), (4, 13)]:
+            T.tnlm_jacobi_step_slab(p, dev(g), dev(g), a, b, ref=dev(ref), f_out=out, variant=T.VARIANT_PAIRED)
+        assert torch.equal(out, got)
 
 
 def test_constant_stack_is_fixed_point_and_bounds(T):
