@@ -13,8 +13,8 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-shared", "--use_fast_math", "-Xptxas", "-v", "-cudart", "static"]
-# --use_fast_math is limited on purpose: the kernels call ex2.approx and divisions explicitly;
-# see DESIGN.md "Arithmetic".
+# --use_fast_math applies to the whole library (flush-to-zero, approximate division and sqrt, also in the
+# metric kernels), "Arithmetic flags", states what depends on it.
 
 
 def sources():
