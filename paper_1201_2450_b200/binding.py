@@ -11,7 +11,7 @@ from __future__ import annotations
 import ctypes as C
 import os
 
-VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED = 0, 1, 2, 3
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED, VARIANT_PAIRED_TMEM = 0, 1, 2, 3, 4
 
 # every symbol include/tnlm.h declares
 EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_jacobi_step",

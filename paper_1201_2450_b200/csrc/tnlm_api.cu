@@ -10,6 +10,7 @@
 #include "tnlm_tiled.cuh"
 #include "tnlm_pair.cuh"
 #include "tnlm_pair5.cuh"
+#include "tnlm_pair_tm.cuh"
 #include "tnlm_metrics.cuh"
 
 namespace {
@@ -64,9 +65,12 @@ int sm_count()
     return n;
 }
 
-int pick_variant(const tnlm_params *p, int variant)
+// ref_is_f: the sweep takes its weights from the stack it averages (TNLM-E); the TMEM kernel covers only that
+int pick_variant(const tnlm_params *p, int variant, bool ref_is_f = true)
 {
     if (variant == TNLM_VARIANT_GENERIC) return TNLM_VARIANT_GENERIC;
+    if (variant == TNLM_VARIANT_PAIRED_TMEM) return (pair_tm_supported(*p) && ref_is_f) ? TNLM_VARIANT_PAIRED_TMEM : -1;
+    if (variant == TNLM_VARIANT_AUTO && pair_tm_supported(*p) && ref_is_f) return TNLM_VARIANT_PAIRED_TMEM;
     if (variant == TNLM_VARIANT_TILED) return tiled_supported(*p) ? TNLM_VARIANT_TILED : -1;
     if (variant == TNLM_VARIANT_PAIRED) return (pair_supported(*p) || pair5_supported(*p)) ? TNLM_VARIANT_PAIRED : -1;
     if (variant == TNLM_VARIANT_AUTO) return (pair_supported(*p) || pair5_supported(*p)) ? TNLM_VARIANT_PAIRED : TNLM_VARIANT_GENERIC;
@@ -79,6 +83,11 @@ int launch_sweep(const tnlm_params *p, const float *f, const float *g, const flo
 {
     if (z1 <= z0) return TNLM_OK;
     const Dims dm = make_dims(*p, z0, z1);
+    if (variant == TNLM_VARIANT_PAIRED_TMEM) {
+        if (ref != f) return TNLM_ERR_UNSUPPORTED;
+        cudaError_t e = launch_pair_tm(*p, dm, f, g, f_out, st);
+        return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "paired (TMEM) sweep launch");
+    }
     if (variant == TNLM_VARIANT_PAIRED) {
         cudaError_t e = p->patch_radius == 2 ? launch_pair5(*p, dm, f, g, ref, f_out, st) : launch_pair(*p, dm, f, g, ref, f_out, st);
         return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "paired sweep launch");
@@ -158,9 +167,9 @@ int tnlm_jacobi_step_slab_variant(const tnlm_params *p, const float *f, const fl
     if (rc) return rc;
     if (!f || !g || !f_out) return TNLM_ERR_NULL_POINTER;
     if (z_begin < 0 || z_end > p->nz || z_begin > z_end) return TNLM_ERR_BAD_DIMS;
-    int v = pick_variant(p, variant);
-    if (v < 0) return TNLM_ERR_UNSUPPORTED;
     if (!ref) ref = f;
+    int v = pick_variant(p, variant, ref == f);
+    if (v < 0) return TNLM_ERR_UNSUPPORTED;
     if (v == TNLM_VARIANT_TILED && ref != f) {   // the scalar tiled kernel covers TNLM-E (ref = f) only
         if (variant != TNLM_VARIANT_AUTO) return TNLM_ERR_UNSUPPORTED;
         v = TNLM_VARIANT_GENERIC;
@@ -446,6 +455,7 @@ const char *tnlm_strerror(int code)
 const char *tnlm_kernel_name(const tnlm_params *p)
 {
     if (check_params(p) != TNLM_OK) return "invalid";
+    if (pair_tm_supported(*p)) return pair_tm_name(*p);
     if (pair5_supported(*p)) return pair5_name(*p);
     return pair_supported(*p) ? pair_name(*p) : "jacobi_generic_kernel";
 }

@@ -30,6 +30,8 @@ def variants(T, p):
             out.append(T.VARIANT_TILED)
         if p.patch_radius in (1, 2):
             out.append(T.VARIANT_PAIRED)
+        if p.patch_radius == 1 and p.search_radius == 2:
+            out.append(T.VARIANT_PAIRED_TMEM)
     return out
 
 
