@@ -14,7 +14,8 @@ seeded synthetic thorax stack.  The metric is BASELINE.json's: voxel-offset upda
 
 `--impl reference` times the CPU oracle (the only "reference implementation" this paper has) and
 prints the same line with "impl": "reference".  Multi-GPU: whole stacks are sharded over ranks
-(independent scans), no data-path collective -> "scaling": "weak".
+(independent scans), no data-path collective -> "scaling": "weak".  `--scaling strong` instead splits ONE
+stack into z-slabs over the ranks (halo exchange per sweep) and prints "scaling": "strong".
 """
 from __future__ import annotations
 
@@ -48,12 +49,19 @@ def parse_args():
     ap.add_argument("--config", default="config3",
                     help="config1..config4: one enhancement per step; config5: the (patch, window) sweep of "
                          "BASELINE.json configs[4], one step = the eight enhancements, per-point figures in 'points'")
-    ap.add_argument("--variant", type=int, default=0, help="kernel variant: 0 auto, 1 generic, 2 tiled, 3 paired")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant: 0 auto, 1 generic, 2 tiled, 3 paired (shared memory), 4 paired with TMEM operands")
     ap.add_argument("--ref", default="same", choices=["same", "separate"],
                     help="separate: every sweep takes its weights from a second stack (tnlm_jacobi_step(ref=...), "
                          "the TNLM-R form of the call, PAPER.md:198) instead of from the iterate; no e2e leg")
     ap.add_argument("--metrics", action="store_true",
                     help="also evaluate the paper's SRR (Eq. 10) and CNR on the enhanced stack and time the TV kernel")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: one independent stack per GPU (the contract's line); strong: ONE stack split into z-slabs "
+                         "over the ranks, each storing slab + halo only, halo exchange per sweep (dist.enhance_z_slabs_local)")
+    ap.add_argument("--loopback-world", type=int, default=0,
+                    help="with --scaling strong on ONE GPU: time the slab of every rank of a W-rank split one after the other "
+                         "(halo planes filled locally, no exchange) and print the slowest rank's time: the compute side of the "
+                         "strong-scaling curve, not a multi-GPU measurement")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -286,6 +294,126 @@ def quality_metrics(T, torch, cfg, g, f):
             "roi": roi, "roi_bg": bg}
 
 
+def run_strong(args, cfg, T, D, info, dev, peaks):
+    """ONE stack of `cfg` split into z-slabs over the ranks: a step is one
+    TNLM-E run through dist.enhance_z_slabs_local with tnlm_jacobi_step_slab as the slab sweep.  Device-timed with
+    CUDA events, max over ranks; value = the one stack's updates / that time."""
+    import torch
+    from tnlm_inputs import make_stack
+    g_np = make_stack(cfg)                                     # every rank paints the same stack and keeps its slab
+    p = T.TnlmParams.make(cfg.shape, cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+    P, Z, Y, X = cfg.shape
+    halo, zt = cfg.search_radius + cfg.patch_radius, T.z_tile(p)
+    L = D.slab_layout(Z, info.rank, info.world, halo, zt)
+    g_own = torch.from_numpy(g_np[:, L.a:L.b].copy()).to(dev)
+    p_loc = T.TnlmParams.make((P, L.nz_local, Y, X), cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+    ws = torch.empty(T.workspace_bytes(p_loc), dtype=torch.uint8, device=dev)
+    launches = [0]
+
+    def sweep_slab(f, g, z0, z1, out):
+        if z1 > z0:
+            T.tnlm_jacobi_step_slab(p_loc, f, g, z0, z1, f_out=out, ws=ws, variant=args.variant)
+            launches[0] += 1
+
+    def step():
+        return D.enhance_z_slabs_local(info, g_own, cfg.n_iter, halo, zt, Z, sweep_slab)
+
+    if args.loopback_world > 0:
+        return run_loopback(args, cfg, T, D, dev, peaks, g_np)
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
+        f, _ = step()
+    torch.cuda.synchronize()
+    if info.world == 1:                                         # the split form must reproduce tnlm_enhance bit for bit
+        want = T.tnlm_enhance(p, torch.from_numpy(g_np).to(dev), cfg.n_iter)
+        assert torch.equal(f.owned(), want), "z-slab form and tnlm_enhance disagree"
+        del want
+    sampler = ClockSampler(info.local_rank)
+    if info.rank == 0:
+        sampler.start()
+    D.barrier(info)
+    torch.cuda.synchronize()
+    launches[0] = 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    D.barrier(info)
+    ms = D.max_over_ranks(info, e0.elapsed_time(e1), device=dev)
+    clocks = sampler.stop() if info.rank == 0 else None
+    halo_bytes = D.sum_over_ranks(info, D.halo_bytes_per_sweep(L, info, (P, Y, X)), device=dev)
+    if info.rank == 0:
+        updates = cfg.updates_per_sweep * cfg.n_iter
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        A = 5 + 6 * cfg.patch_radius
+        value = args.steps * updates / (ms * 1e-3)
+        conf = workload_config(cfg, info.world)
+        conf["workload"] = conf["workload"].replace("+rank", "")
+        conf["parallelism"] = (f"z{info.world}: one stack split into {info.world} z-slabs, each rank stores slab + {halo} halo planes "
+                               f"(+ tile-alignment padding); per sweep the boundary planes go to the z-neighbours by send/recv on a "
+                               f"side stream while the interior is computed")
+        conf["updates_per_step_per_gpu"] = updates / info.world
+        conf["halo_bytes_per_sweep_all_ranks"] = int(halo_bytes)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": info.world, "steps": args.steps, "warmup": warmup,
+                "ms_per_step": ms / args.steps, "s_per_enhancement": ms * 1e-3 / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": conf,
+                "clocks": clocks, "e2e": None, "gpu_launches": launches[0],
+                "roofline": {"bound": "alu", "kernel": kernel_label(T, p, args.variant),
+                             "achieved": value * A / 1e12, "peak": info.world * sms * SM_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12,
+                             "unit": "Tslot/s over all ranks", "frac": value * A / (info.world * sms * SM_LANES * peaks["sm_max_mhz"] * 1e6),
+                             "traffic": None},
+                "cpu_baseline": None, "impl": "tnlm", "kernel": kernel_label(T, p, args.variant), "variant": args.variant}
+        print(json.dumps(line), flush=True)
+    D.finalize(info)
+    return 0
+
+
+def run_loopback(args, cfg, T, D, dev, peaks, g_np):
+    """Compute side of the strong-scaling curve on one GPU: for each rank of a W-rank z-slab split, the time of its
+    sweeps (boundary + interior launches on its local arrays) with the halo planes filled from its own data instead of
+    an exchange.  The slowest rank bounds the job; the exchange (halo bytes below) is not included."""
+    import torch
+    W = args.loopback_world
+    P, Z, Y, X = cfg.shape
+    p = T.TnlmParams.make(cfg.shape, cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+    halo, zt = cfg.search_radius + cfg.patch_radius, T.z_tile(p)
+    rows = []
+    for rank in range(W):
+        info = D.RankInfo(rank, 0, W)
+        L = D.slab_layout(Z, rank, W, halo, zt)
+        g_own = torch.from_numpy(g_np[:, L.a:L.b].copy()).to(dev)
+        p_loc = T.TnlmParams.make((P, L.nz_local, Y, X), cfg.patch_radius, cfg.search_radius, cfg.h, cfg.mu)
+        ws = torch.empty(T.workspace_bytes(p_loc), dtype=torch.uint8, device=dev)
+
+        def sweep_slab(f, g, z0, z1, out):
+            if z1 > z0:
+                T.tnlm_jacobi_step_slab(p_loc, f, g, z0, z1, f_out=out, ws=ws, variant=args.variant)
+
+        def local_fill(_info, stack, L_):
+            stack[:, L_.lo - L_.halo:L_.lo] = stack[:, L_.lo:L_.lo + 1]
+            stack[:, L_.hi:L_.hi + L_.halo] = stack[:, L_.hi - 1:L_.hi]
+
+        for _ in range(2):
+            D.enhance_z_slabs_local(info, g_own, cfg.n_iter, halo, zt, Z, sweep_slab, exchange=local_fill)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            D.enhance_z_slabs_local(info, g_own, cfg.n_iter, halo, zt, Z, sweep_slab, exchange=local_fill)
+        e1.record()
+        torch.cuda.synchronize()
+        rows.append({"rank": rank, "planes": L.b - L.a, "local_planes": L.nz_local, "ms_per_enhancement": e0.elapsed_time(e1) / args.steps,
+                     "halo_bytes_sent_per_sweep": D.halo_bytes_per_sweep(L, info, (P, Y, X))})
+    slow = max(r["ms_per_enhancement"] for r in rows)
+    print(json.dumps({"loopback_world": W, "config": cfg.name, "kernel": kernel_label(T, p, args.variant),
+                      "slowest_rank_ms_per_enhancement": slow,
+                      "projected_updates_per_s_excluding_exchange": cfg.updates_per_sweep * cfg.n_iter / (slow * 1e-3),
+                      "ranks": rows, "note": "one GPU, ranks timed one after the other, halo planes filled locally"}), flush=True)
+    return 0
+
+
 def main():
     args = parse_args()
     from tnlm_inputs import CONFIGS, make_stack
@@ -308,6 +436,10 @@ def main():
     dev = torch.device("cuda", info.local_rank)
     peaks = measured_peaks()
     warmup = max(args.warmup, 3)
+    if args.scaling == "strong":
+        if sweep_mode or args.ref != "same":
+            raise SystemExit("--scaling strong covers config1..config4 with ref = f")
+        return run_strong(args, cfg, T, D, info, dev, peaks)
 
     # one independent, differently seeded stack per rank (weak scaling)
     rcfg = cfg.scaled(seed=cfg.seed + info.rank)

@@ -183,6 +183,19 @@ const char *tnlm_kernel_name(const tnlm_params *p);
 int32_t tnlm_launches_per_sweep(const tnlm_params *p);
 
 /*
+ * z-tile period of the sweep kernels TNLM_VARIANT_AUTO may select for (d, M) (ref == f or not), 1 for the generic
+ * kernel, 0 if the parameters are invalid.  The tiled kernels cut z into tiles that start at multiples of their tile
+ * depth, and a voxel's result depends (in the last bits) on its position inside the tile.  tnlm_jacobi_step_slab
+ * therefore reproduces a whole-volume sweep bit for bit for any [z_begin, z_end).  A rank of the z-slab partition
+ * that stores only its slab plus M+d halo planes gets the same guarantee by
+ * placing its local plane 0 at a global plane that is a multiple of this period, filling the halo planes beyond the
+ * ends of the global volume with copies of the end planes (= the clamp-to-edge reading of the boundary along z), and
+ * calling tnlm_jacobi_step_slab on the local arrays (nz = local plane count, [z_begin, z_end) = its slab in local
+ * indices): paper_1201_2450_b200/dist.py does exactly that.
+ */
+int32_t tnlm_z_tile(const tnlm_params *p);
+
+/*
  * Measurement aid for the FP32 roofline: enqueues a register-resident FFMA
  * loop on every SM; it executes exactly tnlm_probe_fp32_ffma_count(n_iter) FFMA lane-operations.
  * sink is a device buffer of at least 4 bytes.  Time it with CUDA events on `cuda_stream`.

@@ -17,7 +17,7 @@ VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED, VARIANT_PAIRED_TME
 EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_jacobi_step",
            "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
            "tnlm_enhance_host", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
-           "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
+           "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_z_tile", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
            "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr"]
 
 
@@ -72,6 +72,7 @@ def lib():
         L.tnlm_strerror.argtypes = [C.c_int]; L.tnlm_strerror.restype = C.c_char_p
         L.tnlm_kernel_name.argtypes = [pp]; L.tnlm_kernel_name.restype = C.c_char_p
         L.tnlm_launches_per_sweep.argtypes = [pp]; L.tnlm_launches_per_sweep.restype = i32
+        L.tnlm_z_tile.argtypes = [pp]; L.tnlm_z_tile.restype = i32
         L.tnlm_tv_diff.argtypes = [pp, vp, vp, vp, vp]
         L.tnlm_srr.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp]
         L.tnlm_cnr.argtypes = [pp, vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), vp, vp]
@@ -100,6 +101,11 @@ def weights_bytes(p: TnlmParams) -> int:
 
 def host_workspace_bytes(p: TnlmParams) -> int:
     return int(lib().tnlm_host_workspace_bytes(C.byref(p)))
+
+
+def z_tile(p: TnlmParams) -> int:
+    """z-tile period of the sweep kernels for these parameters (include/tnlm.h: tnlm_z_tile)."""
+    return int(lib().tnlm_z_tile(C.byref(p)))
 
 
 def kernel_name(p: TnlmParams) -> str:

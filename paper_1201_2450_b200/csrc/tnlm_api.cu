@@ -466,6 +466,15 @@ int32_t tnlm_launches_per_sweep(const tnlm_params *p)
     return 1;
 }
 
+int32_t tnlm_z_tile(const tnlm_params *p)
+{
+    if (check_params(p) != TNLM_OK) return 0;
+    // least common multiple of the tile depths in launch_pair / launch_pair5 / launch_pair_tm (ref == f and separate ref)
+    if (pair_supported(*p)) return p->search_radius == 3 ? 6 : 4;     // <1,4> <2,4> <3,6> <4,4>; SEP: 4, 4, 2, 2
+    if (pair5_supported(*p)) return p->search_radius == 1 ? 12 : p->search_radius == 4 ? 2 : 4;   // 6|4, 4|2, 4|2, 2|2
+    return 1;
+}
+
 int tnlm_probe_fp32(int32_t n_iter, float *sink, void *cuda_stream)
 {
     if (!sink) return TNLM_ERR_NULL_POINTER;

@@ -91,6 +91,63 @@ def _worker_enhance(rank, world, port, shape, d, M, h, mu, n_sweeps, out_dir):
     D.finalize(info)
 
 
+def _worker_local(rank, world, port, shape, d, M, h, mu, n_sweeps, z_tile, out_dir):
+    """Slab-local storage: the rank never sees more than its slab of g; halos travel by exchange_slab_halos."""
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    from oracle import tnlm_oracle as O
+    from tnlm_inputs import random_stack
+
+    info = D.init("gloo")
+    P, Z, Y, X = shape
+    a, b = D.z_slab(Z, rank, world)
+    g_own = torch.from_numpy(np.ascontiguousarray(random_stack(shape, 7)[:, a:b]))
+    plane = Y * X
+
+    def sweep_slab(f, gg, z0, z1, out):
+        if z1 <= z0:
+            return
+        ZL = f.shape[1]
+        own = (np.arange(P)[:, None] * ZL * plane + np.arange(z0 * plane, z1 * plane)[None, :]).reshape(-1).astype(np.int64)
+        new = O.jacobi_step_at(f.numpy(), gg.numpy(), d, M, np.float32(h), np.float32(mu), own)
+        out.view(-1)[torch.from_numpy(own)] = torch.from_numpy(new)
+
+    f, L = D.enhance_z_slabs_local(info, g_own, n_sweeps, M + d, z_tile, Z, sweep_slab)
+    assert (L.a, L.b) == (a, b) and L.origin % z_tile == 0 and L.lo >= M + d
+    assert f.data.shape[1] == L.nz_local < Z + 2 * (M + d) + z_tile
+    np.save(os.path.join(out_dir, f"loc{rank}.npy"), f.owned().numpy())
+    assert D.halo_bytes_per_sweep(L, info, (P, Y, X)) == (2 if 0 < rank < world - 1 else 1) * P * (M + d) * Y * X * 4
+    D.barrier(info)
+    D.finalize(info)
+
+
+@pytest.mark.parametrize("world,Z,d,M,z_tile", [(2, 9, 1, 2, 4), (3, 13, 1, 1, 4), (2, 8, 2, 1, 12)])
+def test_slab_local_enhancement_equals_single_process(tmp_path, oracle, world, Z, d, M, z_tile):
+    """Every rank stores only slab + halo (+ tile-alignment padding) and the result still equals TNLM-E on the whole
+    stack bit for bit: halo exchange, end-plane replication and the local/global index maps are right."""
+    import torch.multiprocessing as mp
+    shape, h, mu, n_sweeps = (3, Z, 6, 7), 0.3, 0.7, 3
+    mp.spawn(_worker_local, args=(world, _free_port(), shape, d, M, h, mu, n_sweeps, z_tile, str(tmp_path)),
+             nprocs=world, join=True)
+    from tnlm_inputs import random_stack
+    want = oracle.enhance(random_stack(shape, 7), d, M, np.float32(h), np.float32(mu), n_sweeps)
+    got = np.concatenate([np.load(tmp_path / f"loc{r}.npy") for r in range(world)], axis=1)
+    assert np.array_equal(got, want)
+
+
+def test_slab_layouts():
+    from paper_1201_2450_b200 import dist as D
+    for Z, world, halo, t in ((128, 8, 3, 4), (100, 8, 4, 6), (128, 4, 3, 12), (9, 2, 3, 4), (5, 1, 2, 1)):
+        prev_b = 0
+        for r in range(world):
+            L = D.slab_layout(Z, r, world, halo, t)
+            assert L.a == prev_b and L.origin % t == 0 and halo <= L.lo < halo + t and L.hi - L.lo == L.b - L.a
+            prev_b = L.b
+        assert prev_b == Z
+
+
 def test_enhance_z_slabs_two_ranks_equals_single_process(tmp_path, oracle):
     import torch.multiprocessing as mp
     shape, d, M, h, mu, n_sweeps, world = (3, 9, 6, 7), 1, 2, 0.3, 0.7, 3, 2

@@ -488,3 +488,86 @@ def test_guard_regions_stay_untouched(T, shape, d, M):
         assert (wbuf[:4096] == 0x5A).all() and (wbuf[4096 + wsb:] == 0x5A).all(), f"variant {v}: wrote outside the workspace"
         assert (out[:, :za] == -7.5).all() and (out[:, zb:] == -7.5).all(), f"variant {v}: slab sweep wrote outside its planes"
         assert out[:, za:zb].isfinite().all()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("d,M,world,Z", [(1, 2, 3, 37), (2, 1, 2, 30), (1, 3, 2, 22), (1, 2, 1, 9)])
+def test_slab_local_ranks_reproduce_the_enhancement_bitwise(T, d, M, world, Z):
+    """a rank that stores only its z-slab, the M+d halo planes and the tile-alignment padding
+    (dist.enhance_z_slabs_local + tnlm_jacobi_step_slab on the local arrays) reproduces its planes of tnlm_enhance bit
+    for bit.  One GPU, one rank at a time: the halo planes a neighbour would send are taken from the single-device
+    trajectory (loop-back exchange), which is what the neighbours hold if they are right too."""
+    import torch
+    from paper_1201_2450_b200 import dist as D
+    shape, h, mu, n_iter = (3, Z, 40, 36), 0.25, 0.6, 3
+    P, _, Y, X = shape
+    g = dev(random_stack(shape, 11))
+    p = T.TnlmParams.make(shape, d, M, h, mu)
+    iters = [g]
+    for _ in range(n_iter):
+        iters.append(T.tnlm_jacobi_step(p, iters[-1], g))
+    halo, zt = M + d, T.z_tile(p)
+    for rank in range(world):
+        info = D.RankInfo(rank, 0, world)
+        L = D.slab_layout(Z, rank, world, halo, zt)
+        p_loc = T.TnlmParams.make((P, L.nz_local, Y, X), d, M, h, mu)
+        calls = [0]
+
+        def exchange(_info, stack, L_):
+            ref = iters[calls[0]]
+            calls[0] += 1
+            for zl in list(range(L_.lo - L_.halo, L_.lo)) + list(range(L_.hi, L_.hi + L_.halo)):
+                stack[:, zl] = ref[:, min(max(zl + L_.origin, 0), Z - 1)]      # clamp-to-edge beyond the volume (P4)
+
+        def sweep_slab(f, gg, z0, z1, out):
+            if z1 > z0:
+                T.tnlm_jacobi_step_slab(p_loc, f, gg, z0, z1, f_out=out)
+
+        f, L2 = D.enhance_z_slabs_local(info, g[:, L.a:L.b].contiguous(), n_iter, halo, zt, Z, sweep_slab, exchange=exchange)
+        torch.cuda.synchronize()
+        assert calls[0] == n_iter and (L2.a, L2.b) == (L.a, L.b)
+        assert torch.equal(f.owned(), iters[n_iter][:, L.a:L.b]), f"rank {rank} of {world}: slab differs from the single-device run"
+
+
+def _nccl_worker(rank, world, port, shape, d, M, h, mu, n_iter, out_dir):
+    import os
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    import torch
+    import paper_1201_2450_b200 as T
+    from paper_1201_2450_b200 import dist as D
+    torch.cuda.set_device(rank)
+    info = D.init("nccl")
+    P, Z, Y, X = shape
+    p = T.TnlmParams.make(shape, d, M, h, mu)
+    L = D.slab_layout(Z, rank, world, M + d, T.z_tile(p))
+    g_own = torch.from_numpy(np.ascontiguousarray(random_stack(shape, 11)[:, L.a:L.b])).cuda()
+    p_loc = T.TnlmParams.make((P, L.nz_local, Y, X), d, M, h, mu)
+
+    def sweep_slab(f, gg, z0, z1, out):
+        if z1 > z0:
+            T.tnlm_jacobi_step_slab(p_loc, f, gg, z0, z1, f_out=out)
+
+    f, _ = D.enhance_z_slabs_local(info, g_own, n_iter, M + d, T.z_tile(p), Z, sweep_slab)
+    torch.cuda.synchronize()
+    np.save(os.path.join(out_dir, f"nccl{rank}.npy"), f.owned().cpu().numpy())
+    D.barrier(info)
+    D.finalize(info)
+
+
+@pytest.mark.gpu
+def test_two_gpu_z_slab_enhancement_over_nccl(T, tmp_path):
+    """The same on two GPUs with the real exchange (ncclSend/ncclRecv through torch.distributed); skipped on one GPU."""
+    import socket
+    import torch
+    import torch.multiprocessing as mp
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    shape, d, M, h, mu, n_iter = (4, 40, 64, 48), 1, 2, 0.25, 0.6, 4
+    mp.spawn(_nccl_worker, args=(2, port, shape, d, M, h, mu, n_iter, str(tmp_path)), nprocs=2, join=True)
+    g = dev(random_stack(shape, 11))
+    want = T.tnlm_enhance(T.TnlmParams.make(shape, d, M, h, mu), g, n_iter).cpu().numpy()
+    got = np.concatenate([np.load(tmp_path / f"nccl{r}.npy") for r in range(2)], axis=1)
+    assert np.array_equal(got, want)
