@@ -62,6 +62,10 @@ def parse_args():
                     help="with --scaling strong on ONE GPU: time the slab of every rank of a W-rank split one after the other "
                          "(halo planes filled locally, no exchange) and print the slowest rank's time: the compute side of the "
                          "strong-scaling curve, not a multi-GPU measurement")
+    ap.add_argument("--tnlmr", action="store_true",
+                    help="time the TNLM-R path (include/tnlmr.h) instead: the paper's phantom geometry (PAPER.md:245: 10 phases x "
+                         "128^3 voxels, 30 views per phase, 512^2 detector), analytic ellipsoid projections, a step = one outer "
+                         "iteration (3 CGLS iterations + sweep + clamp); prints its own JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -370,6 +374,54 @@ def run_strong(args, cfg, T, D, info, dev, peaks):
     return 0
 
 
+def run_tnlmr(args, T, dev):
+    """One TNLM-R outer iteration per step at the paper's phantom geometry (context for PAPER.md Table 2: 66.9 s per
+    iteration on a Tesla C1060 with unknown d, M).  Not the north-star metric; reported beside it."""
+    import numpy as np
+    import torch
+    from tnlm_inputs import projections as PJ
+    P, n_cgls, d, M, h, mu = 10, 3, 1, 2, 0.05, 0.5
+    geom = PJ.paper_geometry(128, 30, 512)
+    ang, y, clean = PJ.make_projection_stack(geom, P, noise=0.02, seed=5)
+    g = T.TnlmrGeometry.make(P, geom.vol_shape, geom.n_view, geom.nv, geom.nu, geom.voxel, geom.du, geom.dv, geom.sid, geom.sdd)
+    p = T.TnlmParams.make((P,) + geom.vol_shape, d, M, h, mu)
+    yd = torch.from_numpy(y).to(dev)
+    f = torch.zeros((P,) + geom.vol_shape, dtype=torch.float32, device=dev)
+    out = torch.empty_like(f)
+    ws = torch.empty(T.tnlmr_workspace_bytes(g, p), dtype=torch.uint8, device=dev)
+    proj = torch.empty_like(yd)
+    for _ in range(2):
+        T.tnlmr_reconstruct(g, p, ang, yd, f, 1, n_cgls, f_out=out, ws=ws)
+    torch.cuda.synchronize()
+
+    def timed(fn, n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    ms_iter = timed(lambda: T.tnlmr_reconstruct(g, p, ang, yd, f, 1, n_cgls, f_out=out, ws=ws), args.steps)
+    ms_fp = timed(lambda: T.tnlmr_project(g, ang, f, y=proj), 3)
+    ms_bp = timed(lambda: T.tnlmr_backproject(g, ang, yd, f=out), 3)
+    ms_sweep = timed(lambda: T.tnlm_jacobi_step(p, f, f, f_out=out), 3)
+    rec = T.tnlmr_reconstruct(g, p, ang, yd, f, 7, n_cgls, ws=ws)          # the paper ran 7 iterations (PAPER.md:337)
+    cg = T.tnlmr_cgls(g, ang, yd, torch.zeros_like(f), 7 * n_cgls)
+    cl = torch.from_numpy(clean).to(dev)
+    err = lambda a: float(torch.linalg.vector_norm(a - cl) / torch.linalg.vector_norm(cl))
+    rays = P * geom.n_view * geom.nv * geom.nu
+    print(json.dumps({"workload": "TNLM-R, PAPER.md:245 geometry: 10 phases x 128^3 voxels (0.2 cm), 30 views per phase, 512x512 detector, "
+                                  "analytic ellipsoid projections + noise, start f = 0, 3 CGLS iterations per outer iteration, 3^3 patch, 5^3 window",
+                      "ms_per_outer_iteration": ms_iter, "paper_s_per_iteration_c1060": 66.91,
+                      "ms_project_all_phases": ms_fp, "ms_backproject_all_phases": ms_bp, "ms_tnlm_sweep": ms_sweep,
+                      "rays_per_projection": rays, "grays_per_s_project": rays / (ms_fp * 1e-3) / 1e9,
+                      "rel_error_vs_phantom_after_7_iterations": err(rec), "rel_error_cgls_only_21_iterations": err(cg),
+                      "kernel_launches_per_outer_iteration": 2 + 2 + n_cgls * 8 + 3}), flush=True)
+    return 0
+
+
 def run_loopback(args, cfg, T, D, dev, peaks, g_np):
     """Compute side of the strong-scaling curve on one GPU: for each rank of a W-rank z-slab split, the time of its
     sweeps (boundary + interior launches on its local arrays) with the halo planes filled from its own data instead of
@@ -436,6 +488,10 @@ def main():
     dev = torch.device("cuda", info.local_rank)
     peaks = measured_peaks()
     warmup = max(args.warmup, 3)
+    if args.tnlmr:
+        rc = run_tnlmr(args, T, dev)
+        D.finalize(info)
+        return rc
     if args.scaling == "strong":
         if sweep_mode or args.ref != "same":
             raise SystemExit("--scaling strong covers config1..config4 with ref = f")

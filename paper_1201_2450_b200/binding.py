@@ -18,7 +18,8 @@ EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_j
            "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
            "tnlm_enhance_host", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
            "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_z_tile", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
-           "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr"]
+           "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr",
+           "tnlmr_workspace_bytes", "tnlmr_project", "tnlmr_backproject", "tnlmr_cgls", "tnlmr_reconstruct"]
 
 
 class TnlmParams(C.Structure):
@@ -73,6 +74,12 @@ def lib():
         L.tnlm_kernel_name.argtypes = [pp]; L.tnlm_kernel_name.restype = C.c_char_p
         L.tnlm_launches_per_sweep.argtypes = [pp]; L.tnlm_launches_per_sweep.restype = i32
         L.tnlm_z_tile.argtypes = [pp]; L.tnlm_z_tile.restype = i32
+        gp = C.POINTER(TnlmrGeometry)
+        L.tnlmr_workspace_bytes.argtypes = [gp, pp]; L.tnlmr_workspace_bytes.restype = C.c_size_t
+        L.tnlmr_project.argtypes = [gp, vp, vp, vp, vp, C.c_size_t, vp]; L.tnlmr_project.restype = C.c_int
+        L.tnlmr_backproject.argtypes = [gp, vp, vp, vp, vp, C.c_size_t, vp]; L.tnlmr_backproject.restype = C.c_int
+        L.tnlmr_cgls.argtypes = [gp, vp, vp, vp, i32, vp, C.c_size_t, vp]; L.tnlmr_cgls.restype = C.c_int
+        L.tnlmr_reconstruct.argtypes = [gp, pp, vp, vp, vp, vp, i32, i32, i32, vp, C.c_size_t, vp]; L.tnlmr_reconstruct.restype = C.c_int
         L.tnlm_tv_diff.argtypes = [pp, vp, vp, vp, vp]
         L.tnlm_srr.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp]
         L.tnlm_cnr.argtypes = [pp, vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), vp, vp]
@@ -101,6 +108,96 @@ def weights_bytes(p: TnlmParams) -> int:
 
 def host_workspace_bytes(p: TnlmParams) -> int:
     return int(lib().tnlm_host_workspace_bytes(C.byref(p)))
+
+
+class TnlmrGeometry(C.Structure):
+    """Mirror of ``tnlmr_geometry`` (include/tnlmr.h)."""
+    _fields_ = [("n_phase", C.c_int32), ("nz", C.c_int32), ("ny", C.c_int32), ("nx", C.c_int32),
+                ("n_view", C.c_int32), ("nv", C.c_int32), ("nu", C.c_int32),
+                ("voxel", C.c_float), ("du", C.c_float), ("dv", C.c_float), ("sid", C.c_float), ("sdd", C.c_float)]
+
+    @classmethod
+    def make(cls, n_phase, vol_shape, n_view, nv, nu, voxel, du, dv, sid, sdd):
+        nz, ny, nx = (int(v) for v in vol_shape)
+        return cls(int(n_phase), nz, ny, nx, int(n_view), int(nv), int(nu), float(voxel), float(du), float(dv), float(sid), float(sdd))
+
+    @property
+    def vol_shape(self):
+        return (self.n_phase, self.nz, self.ny, self.nx)
+
+    @property
+    def proj_shape(self):
+        return (self.n_phase, self.n_view, self.nv, self.nu)
+
+
+def _angles(g: TnlmrGeometry, angles):
+    import numpy as np
+    a = np.ascontiguousarray(angles, dtype=np.float64)
+    if a.shape != (g.n_phase, g.n_view):
+        raise TypeError(f"angles must have shape {(g.n_phase, g.n_view)}")
+    return a
+
+
+def _dev_like(t, shape, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise TypeError(f"{name} must be a contiguous float32 CUDA tensor of shape {tuple(shape)}")
+    return t.data_ptr()
+
+
+def tnlmr_workspace_bytes(g: TnlmrGeometry, p: TnlmParams = None) -> int:
+    return int(lib().tnlmr_workspace_bytes(C.byref(g), None if p is None else C.byref(p)))
+
+
+def tnlmr_project(g: TnlmrGeometry, angles, f, y=None, stream=None):
+    """y = P f for every phase (include/tnlmr.h)."""
+    import torch
+    a = _angles(g, angles)
+    with _Call(stream, f, y) as c:
+        if y is None:
+            y = torch.empty(g.proj_shape, dtype=torch.float32, device=f.device)
+        ws = c.workspace(None, tnlmr_workspace_bytes(g))
+        _check(lib().tnlmr_project(C.byref(g), a.ctypes.data, _dev_like(f, g.vol_shape, "f"), _dev_like(y, g.proj_shape, "y"),
+                                   ws.data_ptr(), ws.numel(), c.handle), "tnlmr_project")
+    return y
+
+
+def tnlmr_backproject(g: TnlmrGeometry, angles, y, f=None, stream=None):
+    """f = P^T y for every phase."""
+    import torch
+    a = _angles(g, angles)
+    with _Call(stream, f, y) as c:
+        if f is None:
+            f = torch.empty(g.vol_shape, dtype=torch.float32, device=y.device)
+        ws = c.workspace(None, tnlmr_workspace_bytes(g))
+        _check(lib().tnlmr_backproject(C.byref(g), a.ctypes.data, _dev_like(y, g.proj_shape, "y"), _dev_like(f, g.vol_shape, "f"),
+                                       ws.data_ptr(), ws.numel(), c.handle), "tnlmr_backproject")
+    return f
+
+
+def tnlmr_cgls(g: TnlmrGeometry, angles, y, x, n_iter, ws=None, stream=None):
+    """n_iter CGLS iterations on ||P x - y||^2 per phase, x updated in place (and returned)."""
+    a = _angles(g, angles)
+    with _Call(stream, x, y, ws) as c:
+        ws = c.workspace(ws, tnlmr_workspace_bytes(g))
+        _check(lib().tnlmr_cgls(C.byref(g), a.ctypes.data, _dev_like(y, g.proj_shape, "y"), _dev_like(x, g.vol_shape, "x"), int(n_iter),
+                                ws.data_ptr(), ws.numel(), c.handle), "tnlmr_cgls")
+    return x
+
+
+def tnlmr_reconstruct(g: TnlmrGeometry, p: TnlmParams, angles, y, f_init, n_outer, n_cgls, inner_start=0, f_out=None, ws=None,
+                      stream=None):
+    """TNLM-R: n_outer x {CGLS from f^(k-1); weights from g^(k); one sweep of Eq. 8; clamp}."""
+    import torch
+    a = _angles(g, angles)
+    with _Call(stream, y, f_init, f_out, ws) as c:
+        if f_out is None:
+            f_out = torch.empty_like(f_init)
+        ws = c.workspace(ws, tnlmr_workspace_bytes(g, p))
+        _check(lib().tnlmr_reconstruct(C.byref(g), C.byref(p), a.ctypes.data, _dev_like(y, g.proj_shape, "y"),
+                                       _dev_like(f_init, g.vol_shape, "f_init"), _dev_like(f_out, g.vol_shape, "f_out"), int(n_outer),
+                                       int(n_cgls), int(inner_start), ws.data_ptr(), ws.numel(), c.handle), "tnlmr_reconstruct")
+    return f_out
 
 
 def z_tile(p: TnlmParams) -> int:

@@ -24,6 +24,14 @@ int cuda_fail(cudaError_t e, const char *where)
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
     return TNLM_ERR_CUDA;
 }
+}  // namespace
+
+// the other translation units of the library (tnlmr_api.cu) record their CUDA errors in the same thread-local text
+namespace tnlm {
+int record_cuda_error(cudaError_t e, const char *where) { return cuda_fail(e, where); }
+}
+
+namespace {
 
 constexpr int kMaxPatchRadius = 3;
 constexpr int kMaxSearchRadius = 6;

@@ -19,16 +19,21 @@ def T():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "tnlm.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(tnlm_[a-z0-9_]+)\s*\(", text)))
+    """Every function include/*.h declares (tnlm.h: TNLM-E and metrics; tnlmr.h: TNLM-R)."""
+    syms = set()
+    for name in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        if name.endswith(".h"):
+            text = open(os.path.join(ROOT, "include", name)).read()
+            text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+            syms |= set(re.findall(r"\b(tnlmr?_[a-z0-9_]+)\s*\(", text))
+    return sorted(syms)
 
 
 def test_header_symbols_are_exported(T):
     syms = declared_symbols()
     assert len(syms) >= 14
     for s in syms:
-        assert hasattr(T.lib(), s), f"{s} declared in include/tnlm.h but not exported"
+        assert hasattr(T.lib(), s), f"{s} declared in include/*.h but not exported"
     assert sorted(T.EXPORTS) == syms
 
 
@@ -111,3 +116,22 @@ def test_product_package_does_not_import_oracle():
                 text = open(os.path.join(dirpath, fn)).read()
                 for b in banned:
                     assert b not in text, f"{fn} mentions {b}"
+
+
+def test_tnlmr_argument_errors_are_synchronous(T):
+    """include/tnlmr.h: geometry and pointer errors come back as negative codes without touching a device."""
+    g = T.TnlmrGeometry.make(2, (8, 8, 8), 3, 6, 6, 1.0, 1.5, 1.5, 30.0, 45.0)
+    p = T.TnlmParams.make((2, 8, 8, 8), 1, 1, 0.1, 0.5)
+    assert T.tnlmr_workspace_bytes(g) > 0 and T.tnlmr_workspace_bytes(g, p) > T.tnlmr_workspace_bytes(g)
+    assert T.tnlmr_workspace_bytes(g, T.TnlmParams.make((3, 8, 8, 8), 1, 1, 0.1, 0.5)) == 0          # stack shapes differ
+    bad = T.TnlmrGeometry.make(2, (8, 8, 8), 3, 6, 6, 1.0, 1.5, 1.5, 4.0, 45.0)                      # source inside the volume
+    assert T.tnlmr_workspace_bytes(bad) == 0
+    L = T.lib()
+    ang = (C.c_double * 6)(*[0.1 * k for k in range(6)])
+    fake = 0x1000
+    assert L.tnlmr_project(C.byref(g), ang, None, fake, fake, 1 << 20, None) == -1                   # NULL volume
+    assert L.tnlmr_project(C.byref(bad), ang, fake, fake, fake, 1 << 20, None) == -3                 # bad geometry
+    assert L.tnlmr_cgls(C.byref(g), ang, fake, 0x100000, -1, 0x200000, 1 << 30, None) == -3          # negative iteration count
+    assert L.tnlmr_cgls(C.byref(g), ang, fake, 0x100000, 1, 0x200000, 16, None) == -6                # workspace too small
+    assert L.tnlmr_reconstruct(C.byref(g), C.byref(p), ang, fake, 0x100000, 0x100000, 1, 1, 0, 0x4000000, 1 << 30, None) == -5   # f_out aliases f_init
+    assert L.tnlmr_reconstruct(C.byref(g), C.byref(p), ang, fake, 0x100000, 0x200000, 1, 1, 7, 0x4000000, 1 << 30, None) == -3   # bad inner_start
