@@ -100,9 +100,11 @@ template <int M, int RZ, int TX_, bool BTM> struct PairTmGeom {
 
 // One pass (W consecutive x-offsets at fixed (ty, tz), marching the RZ+2 planes): pair_pass of tnlm_pair.cuh with
 // the -ref_i windows and the (Z, N) sums in TMEM.  ta / tz: TMEM addresses of the thread's a-block / accumulator block.
-template <int RZ, int W, bool CAREFUL, int B_PLANE, bool BTM>
+// NR > 0: the ref_j planes live in a ring of NR shared-memory slots, plane p of the march in slot (s0 + p) mod NR.
+template <int RZ, int W, bool CAREFUL, int B_PLANE, bool BTM, int NR = 0>
 __device__ __forceinline__ unsigned pair_pass_tm(const unsigned ta, const unsigned tacc, const float2 *__restrict__ bRow,
-                                                 const float c2, float2 (&bexp)[BTM ? 1 : RZ][2], const unsigned mask)
+                                                 const float c2, float2 (&bexp)[BTM ? 1 : RZ][2], const unsigned mask,
+                                                 const int s0 = 0)
 {
     constexpr int ACC_W = BTM ? 16 : 8;
     constexpr int NVB = (W + 4) / 2;
@@ -115,7 +117,12 @@ __device__ __forceinline__ unsigned pair_pass_tm(const unsigned ta, const unsign
 #pragma unroll
     for (int p = 0; p < RZ + 2; ++p) {
         float2 b[2 * NVB];
-        load_pairs<NVB>(bRow + p * B_PLANE, b);
+        if constexpr (NR == 0) {
+            load_pairs<NVB>(bRow + p * B_PLANE, b);
+        } else {
+            const int sl = s0 + p;
+            load_pairs<NVB>(bRow + (sl >= NR ? sl - NR : sl) * B_PLANE, b);
+        }
         tm_wait_ld();
         if (p + 1 < RZ + 2) tm_ld8(ta + 8 * (p + 1), av[(p + 1) & 1]);
         if (p + 1 >= 2 && p + 1 < RZ + 2) {
@@ -369,20 +376,6 @@ cudaError_t launch_pair_tm_t(const Dims &dm, const float *f, const float *g, flo
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
     tnlm_pair_tm_kernel<M, RZ, TX_, NCTA, BTM><<<(unsigned)blocks, G::NT, G::BYTES, st>>>(f, g, f_out, dm, tiles_x, tiles_y, tiles_z);
     return cudaGetLastError();
-}
-
-// ---------------------------------------------------------------------------------------------
-inline bool pair_tm_supported(const tnlm_params &p) { return p.patch_radius == 1 && p.search_radius == 2; }
-inline const char *pair_tm_name(const tnlm_params &) { return "tnlm_pair_tm_kernel<M=2>"; }
-
-// ref must be f (TNLM-E); <M, RZ, TX, CTAs per SM, reference exponents in TMEM>
-inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const float *f, const float *g, float *f_out,
-                                  cudaStream_t st)
-{
-    switch (p.search_radius) {
-        case 2: return launch_pair_tm_t<2, 4, 16, 3, true>(dm, f, g, f_out, st);
-        default: return cudaErrorNotSupported;
-    }
 }
 
 }  // namespace tnlm
