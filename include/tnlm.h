@@ -64,9 +64,10 @@ typedef enum {
  *   TILED    d = 1, 1 <= M <= 4, ref == f: scalar FP32 tiles (first optimised kernel, kept for cross-checks)
  *   PAIRED   d = 1 or 2, 1 <= M <= 4, any ref: row-pair packed FP32 (FADD2 / FFMA2) -- what AUTO selects there
  *            (with ref != f the kernel keeps a second neighbour tile for the candidate values: smaller tiles, slower)
- *   PAIRED_TMEM  d = 1, 2 <= M <= 4, ref == f: the PAIRED arithmetic with the thread-private operands (the -ref_i
- *            windows, Z, N and the reference exponents) in Blackwell tensor memory, and for M >= 3 a rolling window of
- *            ref_j planes in shared memory (three / two CTAs per SM instead of one) -- what AUTO selects there
+ *   PAIRED_TMEM  d = 1 or 2, 2 <= M <= 4, ref == f: the PAIRED arithmetic with the thread-private operands (the -ref_i
+ *            windows, Z, N and the reference exponents) in Blackwell tensor memory, and (d = 1: M >= 3; d = 2: all) a
+ *            rolling window of ref_j planes in shared memory (three / two CTAs per SM instead of one or two) -- what
+ *            AUTO selects there
  * A separate ref with TILED or PAIRED_TMEM is refused (TNLM_ERR_UNSUPPORTED). */
 enum { TNLM_VARIANT_AUTO = 0, TNLM_VARIANT_GENERIC = 1, TNLM_VARIANT_TILED = 2, TNLM_VARIANT_PAIRED = 3,
        TNLM_VARIANT_PAIRED_TMEM = 4 };

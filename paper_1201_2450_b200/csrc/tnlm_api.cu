@@ -10,7 +10,7 @@
 #include "tnlm_tiled.cuh"
 #include "tnlm_pair.cuh"
 #include "tnlm_pair5.cuh"
-#include "tnlm_pair_tmr.cuh"
+#include "tnlm_pair5_tm.cuh"
 #include "tnlm_metrics.cuh"
 
 namespace {
@@ -479,7 +479,7 @@ int32_t tnlm_z_tile(const tnlm_params *p)
     if (check_params(p) != TNLM_OK) return 0;
     // least common multiple of the tile depths in launch_pair / launch_pair5 / launch_pair_tm (ref == f and separate ref)
     if (pair_supported(*p)) return p->search_radius == 3 ? 12 : 4;    // <1,4> <2,4> <3,6> <4,4>; TMEM: 4; SEP: 4, 4, 2, 2
-    if (pair5_supported(*p)) return p->search_radius == 1 ? 12 : p->search_radius == 4 ? 2 : 4;   // 6|4, 4|2, 4|2, 2|2
+    if (pair5_supported(*p)) return p->search_radius == 1 ? 12 : 4;   // 6|4, 4|2, 4|2, 2|2; TMEM: 4
     return 1;
 }
 

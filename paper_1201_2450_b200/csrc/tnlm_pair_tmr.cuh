@@ -224,31 +224,4 @@ cudaError_t launch_pair_tmr_t(const Dims &dm, const float *f, const float *g, fl
     return cudaGetLastError();
 }
 
-// ---------------------------------------------------------------------------------------------
-// TNLM_VARIANT_PAIRED_TMEM: whole tile resident at M = 2 (tnlm_pair_tm_kernel), rolling window at M = 3, 4
-inline bool pair_tm_supported(const tnlm_params &p)
-{
-    return p.patch_radius == 1 && p.search_radius >= 2 && p.search_radius <= 4;
-}
-inline const char *pair_tm_name(const tnlm_params &p)
-{
-    switch (p.search_radius) {
-        case 2: return "tnlm_pair_tm_kernel<M=2>";
-        case 3: return "tnlm_pair_tmr_kernel<M=3>";
-        default: return "tnlm_pair_tmr_kernel<M=4>";
-    }
-}
-
-// ref must be f (TNLM-E)
-inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const float *f, const float *g, float *f_out,
-                                  cudaStream_t st)
-{
-    switch (p.search_radius) {
-        case 2: return launch_pair_tm_t<2, 4, 16, 3, true>(dm, f, g, f_out, st);   // <M, RZ, TX, CTAs per SM, b in TMEM>
-        case 3: return launch_pair_tmr_t<3, 4, 3>(dm, f, g, f_out, st);            // <M, RZ, CTAs per SM>
-        case 4: return launch_pair_tmr_t<4, 4, 2>(dm, f, g, f_out, st);
-        default: return cudaErrorNotSupported;
-    }
-}
-
 }  // namespace tnlm

@@ -30,7 +30,7 @@ def variants(T, p):
             out.append(T.VARIANT_TILED)
         if p.patch_radius in (1, 2):
             out.append(T.VARIANT_PAIRED)
-        if p.patch_radius == 1 and 2 <= p.search_radius <= 4:
+        if p.patch_radius in (1, 2) and 2 <= p.search_radius <= 4:
             out.append(T.VARIANT_PAIRED_TMEM)
     return out
 
