@@ -256,6 +256,8 @@ def roofline_block(T, p, cfg, variant, launch_ms, sms, peaks, clocks, probe_slot
                 "peak_gbs": peaks["hbm_gbs"], "frac": alg_bytes / (launch_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                 "peak_source": peaks["source"]},
     }
+    out["issue_model"] = ("packed FP32 instructions hold the issue port for two cycles: the sweep kernels are bound by issue slots "
+                          "(pair_tm at config 3: 18.5 slots per update against A = 11, 0.91 slots per cycle; profiles/r02_issue_model.md)")
     if probe_slots_per_s:
         out["ffma_probe_tslots"] = probe_slots_per_s / 1e12
         out["frac_of_ffma_probe"] = rate * A / probe_slots_per_s
