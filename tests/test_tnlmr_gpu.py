@@ -45,6 +45,8 @@ def dev(a):
 
 
 def geoms(T, R, P, vol, n_view, nv, nu, voxel, du, dv, sid, sdd):
+    """The same geometry for both sides: tnlmr_geometry carries fp32 lengths, so the oracle gets the fp32-rounded values."""
+    voxel, du, dv, sid, sdd = (float(np.float32(v)) for v in (voxel, du, dv, sid, sdd))
     return (T.TnlmrGeometry.make(P, vol, n_view, nv, nu, voxel, du, dv, sid, sdd),
             R.geom(vol, n_view, nu, nv, du, dv, sid, sdd, voxel))
 
@@ -148,3 +150,18 @@ def test_tnlmr_loop_matches_the_oracle(T, R, inner_start):
     if inner_start == 0:
         only_cgls = T.tnlmr_cgls(g, ang, dev(y), dev(f0), n_outer * n_cgls).cpu().numpy()
         assert np.linalg.norm(got - clean) < np.linalg.norm(only_cgls - clean)
+
+
+def test_projector_pair_at_the_papers_geometry(T, R):
+    """One phase at PAPER.md:245's size (128^3 voxels of 0.2 cm, 30 views, 512 x 512 pixels, 100 / 153.6 cm): the launch
+    shape bench.py --tnlmr times, every ray and every voxel against the oracle."""
+    geom = PJ.paper_geometry(128, 30, 512)
+    g, rg = geoms(T, R, 1, geom.vol_shape, geom.n_view, geom.nv, geom.nu, geom.voxel, geom.du, geom.dv, geom.sid, geom.sdd)
+    rng = np.random.default_rng(12)
+    ang = PJ.phase_angles(10, 30)[3:4]
+    f = rng.random((1,) + geom.vol_shape).astype(np.float32)
+    y = rng.standard_normal((1, 30, 512, 512)).astype(np.float32)
+    m, l2 = rel(T.tnlmr_project(g, ang, dev(f)).cpu().numpy()[0], R.project(rg, ang[0], f[0]))
+    assert m <= 2e-5 and l2 <= 1e-5, f"project: {m:.2e} {l2:.2e}"
+    m, l2 = rel(T.tnlmr_backproject(g, ang, dev(y)).cpu().numpy()[0], R.backproject(rg, ang[0], y[0]))
+    assert m <= 2e-5 and l2 <= 1e-5, f"backproject: {m:.2e} {l2:.2e}"
