@@ -93,20 +93,28 @@ __global__ void __launch_bounds__(128) siddon_kernel(const RGeom g, const double
         setup(2, iz, sz, az, dz);
         const float yr = BACK ? y_in[ybase] : 0.f;
         double ac = amin;
-        const int guard = g.X + g.Y + g.Z + 4;
-        for (int it = 0; it < guard && ac < amax; ++it) {
-            const double am = fmin(ax, fmin(ay, az));
-            const double an = fmax(ac, fmin(am, amax));   // a crossing that rounding put before the entry must not move the walk back
-            const float len = (float)((an - ac) * L);
-            if (len > 0.f) {
-                const size_t vi = vbase + ((size_t)iz * g.Y + iy) * g.X + ix;
+        size_t vi = vbase + ((size_t)iz * g.Y + iy) * g.X + ix;
+        const ptrdiff_t stx = sx, sty = (ptrdiff_t)sy * g.X, stz = (ptrdiff_t)sz * g.Y * g.X;
+        // one segment per iteration: the nearest crossing ends it (a crossing that rounding put before the entry must
+        // not move the walk back; the exit parameter ends the last one); branches instead of 64-bit selects
+        for (int it = g.X + g.Y + g.Z + 4; it > 0; --it) {
+            double an;
+            int axis;
+            if (ax <= ay && ax <= az) { an = ax; axis = 0; }
+            else if (ay <= az) { an = ay; axis = 1; }
+            else { an = az; axis = 2; }
+            const bool last = !(an < amax);
+            if (last) an = amax;
+            if (an > ac) {
+                const float len = (float)((an - ac) * L);
                 if (BACK) atomicAdd(vol_out + vi, len * yr);
                 else acc = fmaf(len, __ldg(vol_in + vi), acc);
+                ac = an;
             }
-            ac = an;
-            if (ax <= ay && ax <= az) { ix += sx; ax += dx; if (ix < 0 || ix >= g.X) break; }
-            else if (ay <= az) { iy += sy; ay += dy; if (iy < 0 || iy >= g.Y) break; }
-            else { iz += sz; az += dz; if (iz < 0 || iz >= g.Z) break; }
+            if (last) break;
+            if (axis == 0) { ix += sx; ax += dx; vi += stx; if ((unsigned)ix >= (unsigned)g.X) break; }
+            else if (axis == 1) { iy += sy; ay += dy; vi += sty; if ((unsigned)iy >= (unsigned)g.Y) break; }
+            else { iz += sz; az += dz; vi += stz; if ((unsigned)iz >= (unsigned)g.Z) break; }
         }
     }
     if (!BACK) y_out[ybase] = acc;
