@@ -382,11 +382,15 @@ int tnlm_tv_diff(const tnlm_params *p, const float *a, const float *b, double *t
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaMemsetAsync(tv_out, 0, sizeof(double) * p->n_phase, st);
     if (e != cudaSuccess) return cuda_fail(e, "tv memset");
-    const size_t groups = (size_t)p->nz * p->ny * ((p->nx + 3) / 4);
-    size_t blocks = (groups + kMetricThreads - 1) / kMetricThreads;
-    const size_t cap = (size_t)sm_count() * 16 / (size_t)p->n_phase + 1;   // ~16 CTAs (two full waves of 8) per SM over all phases
-    if (blocks > cap) blocks = cap;
-    tv_diff_kernel<<<dim3((unsigned)blocks, (unsigned)p->n_phase), kMetricThreads, 0, st>>>(a, b, tv_out, p->nz, p->ny, p->nx);
+    const int xq = (p->nx + 3) / 4;
+    const int XQ = xq > 32 ? 64 : xq > 16 ? 32 : 16;                 // x-quads per CTA row
+    const int tiles_xq = (xq + XQ - 1) / XQ, tiles_y = (p->ny + kMetricThreads / XQ - 1) / (kMetricThreads / XQ);
+    const long long blocks = (long long)tiles_xq * tiles_y * ((p->nz + kTvZChunk - 1) / kTvZChunk);
+    if (blocks > 2147483647LL) return TNLM_ERR_BAD_DIMS;
+    const dim3 grid((unsigned)blocks, (unsigned)p->n_phase);
+    if (XQ == 64) tv_diff_kernel<64><<<grid, kMetricThreads, 0, st>>>(a, b, tv_out, p->nz, p->ny, p->nx, tiles_xq, tiles_y);
+    else if (XQ == 32) tv_diff_kernel<32><<<grid, kMetricThreads, 0, st>>>(a, b, tv_out, p->nz, p->ny, p->nx, tiles_xq, tiles_y);
+    else tv_diff_kernel<16><<<grid, kMetricThreads, 0, st>>>(a, b, tv_out, p->nz, p->ny, p->nx, tiles_xq, tiles_y);
     e = cudaGetLastError();
     return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "tv launch");
 }

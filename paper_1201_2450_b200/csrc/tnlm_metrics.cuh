@@ -51,49 +51,61 @@ __device__ __forceinline__ void load_h4(const float *__restrict__ ap, const floa
 }
 
 // tv[p] += sum over the voxels of phase p of |grad (a - b)| (forward differences, 0 across the boundary).
-// grid = (blocks per phase, P); a thread handles 4 consecutive x of a row per step: its own quad, the quad
-// one row down and the quad one plane down (float4 loads when nx % 4 == 0), plus one scalar for the x-difference
-// of its last voxel.  Per-voxel arithmetic in fp32 (each |grad h| is good to ~3 ulp = 2e-7 relative, and the
-// terms are non-negative, so the sum inherits that bound: DESIGN.md M4), accumulation in fp64: with fp64
-// differences and DSQRT the kernel is bound by the FP64 pipe at a quarter of the HBM roofline.
+// A CTA is a tile of kTvXQ x-quads x 256/kTvXQ rows that marches kTvZChunk planes: a thread handles 4 consecutive x of one row
+// and keeps the next plane's quad in registers, so the plane-down difference costs no second read; the row-down quad
+// and the scalar right of the quad are re-reads inside the CTA's own tile (L1) except at its last row.  Every voxel
+// thus crosses L2 about 1.3 times (the first, grid-stride form read every operand three times from L2 and was bound
+// by it at 0.4 of the HBM roofline).  Per-voxel arithmetic in fp32 (each |grad h| is good to ~3 ulp = 2e-7 relative,
+// and the terms are non-negative, so the sum inherits that bound: DESIGN.md M4), accumulation in fp64.
+constexpr int kTvZChunk = 16;
+
+template <int kTvXQ>   // x-quads per CTA row: 64, or fewer for narrow volumes so that no thread idles
 __global__ void __launch_bounds__(kMetricThreads)
 tv_diff_kernel(const float *__restrict__ a, const float *__restrict__ b, double *__restrict__ tv, const int Z,
-               const int Y, const int X)
+               const int Y, const int X, const int tiles_xq, const int tiles_y)
 {
+    constexpr int kTvRows = kMetricThreads / kTvXQ;
     const int ph = blockIdx.y;
     const size_t V = (size_t)Z * Y * X;
     const float *ap = a + ph * V;
     const float *bp = b ? b + ph * V : nullptr;
-    const int xq = (X + 3) / 4;                        // groups of 4 voxels per row
-    const unsigned groups = (unsigned)Z * Y * xq;     // < 2^31: a stack has at most 2^31 - 1 voxels (32-bit index math)
+    int t = blockIdx.x;
+    const int bxq = t % tiles_xq; t /= tiles_xq;
+    const int by = t % tiles_y; t /= tiles_y;
+    const int z0 = t * kTvZChunk, z1 = min(z0 + kTvZChunk, Z);
+    const int xg = bxq * kTvXQ + (threadIdx.x % kTvXQ), y = by * kTvRows + threadIdx.x / kTvXQ;
     const bool vec = (X % 4) == 0;
     double acc[1] = {0.0};
-    for (unsigned gi = blockIdx.x * blockDim.x + threadIdx.x; gi < groups; gi += gridDim.x * blockDim.x) {
-        const unsigned row = gi / xq;
-        const int xg = (int)(gi - row * xq);
-        const int z = (int)(row / Y), y = (int)(row - (unsigned)z * Y);
-        const size_t base = (size_t)row * X + 4 * xg;
+    if (4 * xg < X && y < Y) {
         const int n = min(4, X - 4 * xg);
-        float c[4], cy[4], cz[4];
+        const bool has_y = y + 1 < Y, has_next = 4 * xg + n < X;
+        const size_t plane = (size_t)Y * X;
+        size_t base = ((size_t)z0 * Y + y) * X + 4 * xg;
+        float c[4], cz[4];
         load_h4(ap, bp, base, n, vec, c);
-        const bool has_y = y + 1 < Y, has_z = z + 1 < Z;
-        if (has_y) load_h4(ap, bp, base + X, n, vec, cy);
-        if (has_z) load_h4(ap, bp, base + (size_t)Y * X, n, vec, cz);
-        float cnext = 0.f;                             // h at x + n (first voxel of the next quad), if inside the row
-        if (4 * xg + n < X) cnext = __ldg(ap + base + n) - (bp ? __ldg(bp + base + n) : 0.f);
-        float quad = 0.f;
+        for (int z = z0; z < z1; ++z, base += plane) {
+            const bool has_z = z + 1 < Z;
+            float cy[4];
+            if (has_z) load_h4(ap, bp, base + plane, n, vec, cz);
+            if (has_y) load_h4(ap, bp, base + X, n, vec, cy);
+            float cnext = 0.f;                         // h at x + n (first voxel of the next quad), if inside the row
+            if (has_next) cnext = __ldg(ap + base + n) - (bp ? __ldg(bp + base + n) : 0.f);
+            float quad = 0.f;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (k < n) {
-                const bool last_x = (4 * xg + k == X - 1);
-                const float nx = (k + 1 < n) ? c[(k + 1) & 3] : cnext;
-                const float gx = last_x ? 0.f : nx - c[k];
-                const float gy = has_y ? cy[k] - c[k] : 0.f;
-                const float gz = has_z ? cz[k] - c[k] : 0.f;
-                quad += sqrtf(fmaf(gx, gx, fmaf(gy, gy, gz * gz)));
+            for (int k = 0; k < 4; ++k) {
+                if (k < n) {
+                    const bool last_x = (4 * xg + k == X - 1);
+                    const float nx = (k + 1 < n) ? c[(k + 1) & 3] : cnext;
+                    const float gx = last_x ? 0.f : nx - c[k];
+                    const float gy = has_y ? cy[k] - c[k] : 0.f;
+                    const float gz = has_z ? cz[k] - c[k] : 0.f;
+                    quad += sqrtf(fmaf(gx, gx, fmaf(gy, gy, gz * gz)));
+                }
             }
+            acc[0] += (double)quad;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) c[k] = cz[k];
         }
-        acc[0] += (double)quad;
     }
     block_accumulate<1>(acc, tv + ph);
 }
