@@ -554,6 +554,59 @@ def _nccl_worker(rank, world, port, shape, d, M, h, mu, n_iter, out_dir):
     D.finalize(info)
 
 
+def _gloo_cuda_worker(rank, world, port, shape, d, M, h, mu, n_iter, out_dir):
+    import os
+    os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    import torch
+    import paper_1201_2450_b200 as T
+    from paper_1201_2450_b200 import dist as D
+    torch.cuda.set_device(0)
+    info = D.init("gloo")
+    P, Z, Y, X = shape
+    p = T.TnlmParams.make(shape, d, M, h, mu)
+    L = D.slab_layout(Z, rank, world, M + d, T.z_tile(p))
+    g_own = torch.from_numpy(np.ascontiguousarray(random_stack(shape, 11)[:, L.a:L.b])).cuda()
+    p_loc = T.TnlmParams.make((P, L.nz_local, Y, X), d, M, h, mu)
+
+    def sweep_slab(f, gg, z0, z1, out):
+        if z1 > z0:
+            T.tnlm_jacobi_step_slab(p_loc, f, gg, z0, z1, f_out=out)
+
+    def exchange_via_host(info_, stack, L_):
+        # gloo cannot send CUDA memory: stage the local array through the host on whatever stream is current (the side
+        # stream inside enhance_z_slabs_local), run the library's exchange on the copy, write the halo planes back
+        host = stack.cpu()
+        D.exchange_slab_halos(info_, host, L_)
+        h = L_.halo
+        stack[:, L_.lo - h:L_.lo].copy_(host[:, L_.lo - h:L_.lo])
+        stack[:, L_.hi:L_.hi + h].copy_(host[:, L_.hi:L_.hi + h])
+
+    f, _ = D.enhance_z_slabs_local(info, g_own, n_iter, M + d, T.z_tile(p), Z, sweep_slab, exchange=exchange_via_host)
+    torch.cuda.synchronize()
+    np.save(os.path.join(out_dir, f"gc{rank}.npy"), f.owned().cpu().numpy())
+    D.barrier(info)
+    D.finalize(info)
+
+
+@pytest.mark.gpu
+def test_two_rank_z_slab_enhancement_with_a_real_exchange_on_one_gpu(T, tmp_path):
+    """Two processes share cuda:0 and exchange their halo planes through torch.distributed (gloo, staged through the
+    host): the device side of dist.enhance_z_slabs_local -- side stream, events, boundary / interior launches on
+    slab-local arrays -- with a real neighbour, bit-identical to tnlm_enhance.  A correctness test only: nothing is
+    timed with two ranks on one GPU."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    shape, d, M, h, mu, n_iter = (3, 26, 40, 36), 1, 2, 0.25, 0.6, 3
+    mp.spawn(_gloo_cuda_worker, args=(2, port, shape, d, M, h, mu, n_iter, str(tmp_path)), nprocs=2, join=True)
+    g = dev(random_stack(shape, 11))
+    want = T.tnlm_enhance(T.TnlmParams.make(shape, d, M, h, mu), g, n_iter).cpu().numpy()
+    got = np.concatenate([np.load(tmp_path / f"gc{r}.npy") for r in range(2)], axis=1)
+    assert np.array_equal(got, want)
+
+
 @pytest.mark.gpu
 def test_two_gpu_z_slab_enhancement_over_nccl(T, tmp_path):
     """The same on two GPUs with the real exchange (ncclSend/ncclRecv through torch.distributed); skipped on one GPU."""
