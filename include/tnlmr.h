@@ -18,8 +18,10 @@
  *
  * Layout: volumes are [phase][z][y][x] fp32 stacks (as in tnlm.h), projections [phase][view][v][u] fp32; both DEVICE
  * pointers, 16-byte aligned, owned by the caller.  `angles` is a HOST pointer to n_phase * n_view doubles (radians,
- * [phase][view]); it is read before the call returns.  Every phase has n_view views.  Calls enqueue work on
- * `cuda_stream` and return; argument errors are synchronous negative tnlm_status codes (tnlm.h).
+ * [phase][view]); it is read before the call returns.  Every phase has n_view views.  Every call first uploads the
+ * (cos, sin) table of the angles and waits for that copy on `cuda_stream` (one stream synchronisation, so work queued
+ * earlier on the stream has finished too); the kernels are then enqueued and the call returns.  Argument errors are
+ * synchronous negative tnlm_status codes (tnlm.h).
  * The back-projector and the dot products of CGLS accumulate with atomic adds, so results are reproducible to
  * rounding, not bit for bit.
  */
