@@ -129,11 +129,11 @@ int tnlm_enhance_variant(const tnlm_params *p, const float *g, const float *f_in
  * End-to-end form of tnlm_enhance for HOST buffers: g_host / f_init_host (may be NULL) / f_out_host
  * are host pointers (pinned memory makes the copies asynchronous).  The call copies the inputs to the
  * device, runs tnlm_enhance and copies the result back, all on `cuda_stream`, then synchronises the
- * stream before returning.  For f_init_host == NULL, n_iter >= 1 and volumes deep enough for four z-slabs
- * (nz >= 32 and 8 * floor(nz / 32) >= M + d + 8) the copies are pipelined: the
- * stack travels in four z-slabs on a copy stream that the call creates and destroys, the first sweep starts on the
- * slabs that have arrived and the last sweep returns its slabs as they finish (same bits as the plain path: slab
- * sweeps reproduce the whole-volume sweep exactly).  dev_ws is a caller-owned DEVICE workspace of at least
+ * stream before returning.  For f_init_host == NULL, n_iter >= 1 and nz >= 32 the copies are pipelined: the
+ * stack travels in z-slabs of 8, 16, 32, ... planes on a copy stream that the call creates and destroys, the first
+ * sweep starts on the slabs that have arrived (with the M + d planes of halo beyond them) and the last sweep returns
+ * its slabs, largest first, as they finish (same bits as the plain path: slab sweeps reproduce the whole-volume
+ * sweep exactly).  dev_ws is a caller-owned DEVICE workspace of at least
  * tnlm_host_workspace_bytes(p) bytes (it holds the device stacks as well as the kernel workspace).
  */
 size_t tnlm_host_workspace_bytes(const tnlm_params *p);

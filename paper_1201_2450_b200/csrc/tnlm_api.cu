@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 #include "tnlm_common.cuh"
 #include "tnlm_generic.cuh"
@@ -258,41 +259,74 @@ int tnlm_enhance(const tnlm_params *p, const float *g, const float *f_init, floa
     return tnlm_enhance_variant(p, g, f_init, f_out, n_iter, ws, ws_bytes, cuda_stream, TNLM_VARIANT_AUTO);
 }
 
-// Pipelined form of tnlm_enhance_host (f_init == g, n_iter >= 1, volumes deep enough for four z-slabs): the stack
-// goes to the device slab by slab on an internal copy stream while the first sweep already runs on the slabs whose
-// planes (and M+d planes of halo) have arrived, and the last sweep hands its slabs back the same way.  Slab sweeps
+// Slab bounds of the pipelined host path.  A slab of the first sweep can start once its planes and `look` planes
+// beyond them are on the device, and the copy runs about twice as fast as the 5^3-window sweep, so the slabs double:
+// [0, 8) [8, 24) [24, 56) [56, 120) ... keep the kernel one slab behind the copy after a start-up of 8 + look planes.
+// The last sweep mirrors the bounds (... 32, 16, 8 planes): each slab's way back overlaps the sweeps of the smaller
+// slabs after it and only the last 8 planes are exposed.  A single sweep (first and last at once) takes 16-plane slabs.
+static std::vector<int> slab_bounds(const int nz, const bool grow, const bool shrink)
+{
+    std::vector<int> zb{0};
+    if (grow && shrink) {
+        const int step = std::max(16, (nz + 11) / 12 / 8 * 8);
+        for (int z = step; z < nz; z += step) zb.push_back(z);
+    } else {
+        std::vector<int> cut;
+        for (int z = 8; z < nz; z = 2 * z + 8) cut.push_back(z);
+        if (grow) {
+            zb.insert(zb.end(), cut.begin(), cut.end());
+        } else {
+            for (auto it = cut.rbegin(); it != cut.rend(); ++it) {
+                const int z = (nz - *it) / 8 * 8;
+                if (z > zb.back()) zb.push_back(z);
+            }
+        }
+    }
+    zb.push_back(nz);
+    return zb;
+}
+
+// Pipelined form of tnlm_enhance_host (f_init == g, n_iter >= 1, nz >= 32): the stack goes to the device in z-chunks
+// on an internal copy stream while the first sweep already runs on the slabs whose planes (and the planes their last
+// z-tile and the M+d halo reach into) have arrived, and the last sweep hands its slabs back the same way.  Slab sweeps
 // are bit-identical to whole-volume sweeps (z-tiles are aligned to absolute plane indices), so the result equals
 // tnlm_enhance's bit for bit.
 static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, float *f_out_host, int32_t n_iter,
                                   float *g_dev, float *fo_dev, void *ws, size_t ws_bytes, cudaStream_t st, int variant)
 {
-    constexpr int NS = 4;
-    constexpr int kMaxRZ = 8;   // deepest z-tile of any sweep kernel (tiles are aligned to absolute multiples of RZ)
-    const int halo = p->search_radius + p->patch_radius;
+    // planes past its end that a slab's sweep reads: the halo, and the rest of a z-tile that straddles the bound
+    // (bounds are multiples of 8; the deepest tile of any sweep kernel is 8 planes)
+    const int zt = tnlm_z_tile(p);
+    const int look = p->search_radius + p->patch_radius + ((zt > 0 && 8 % zt == 0) ? 0 : 7);
     const size_t plane = (size_t)p->ny * p->nx, pitch = plane * p->nz * sizeof(float), sb = stack_bytes(p);
-    int zb[NS + 1];
-    for (int s = 0; s <= NS; ++s) zb[s] = (int)((long long)p->nz * s / NS) / 8 * 8;   // slab bounds on multiples of 8
-    zb[NS] = p->nz;
+    const std::vector<int> zin = slab_bounds(p->nz, true, n_iter == 1);
+    const std::vector<int> zout = n_iter == 1 ? zin : slab_bounds(p->nz, false, true);
+    const int n_in = (int)zin.size() - 1, n_out = (int)zout.size() - 1;
     cudaStream_t cs = nullptr;
-    cudaEvent_t ev_in[NS] = {}, ev_out[NS] = {}, ev_start = nullptr;
+    std::vector<cudaEvent_t> ev_in(n_in, nullptr), ev_out(n_out, nullptr);
+    cudaEvent_t ev_start = nullptr;
     cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
     if (e != cudaSuccess) return cuda_fail(e, "copy stream");
     int rc = TNLM_OK;
     auto fail = [&](cudaError_t err, const char *what) { rc = cuda_fail(err, what); };
     auto ck = [&](cudaError_t err, const char *what) { if (err != cudaSuccess && rc == TNLM_OK) fail(err, what); return err == cudaSuccess; };
     ck(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming), "event");
-    for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
-        ck(cudaEventCreateWithFlags(&ev_in[s], cudaEventDisableTiming), "event");
-        ck(cudaEventCreateWithFlags(&ev_out[s], cudaEventDisableTiming), "event");
-    }
+    for (int s = 0; s < n_in && rc == TNLM_OK; ++s) ck(cudaEventCreateWithFlags(&ev_in[s], cudaEventDisableTiming), "event");
+    for (int s = 0; s < n_out && rc == TNLM_OK; ++s) ck(cudaEventCreateWithFlags(&ev_out[s], cudaEventDisableTiming), "event");
     if (rc == TNLM_OK) {
-        // the copy stream starts after whatever the caller queued on its stream before this call
+        // the copy stream starts after whatever the caller queued on its stream before this call; chunk s ends where
+        // slab s of the first sweep stops reading, so ev_in[s] is all that slab waits for
         ck(cudaEventRecord(ev_start, st), "event record");
         ck(cudaStreamWaitEvent(cs, ev_start, 0), "stream wait");
-        for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
-            const size_t off = (size_t)zb[s] * plane;
-            ck(cudaMemcpy2DAsync(g_dev + off, pitch, g_host + off, pitch, (size_t)(zb[s + 1] - zb[s]) * plane * sizeof(float),
-                                 (size_t)p->n_phase, cudaMemcpyHostToDevice, cs), "H2D slab");
+        int z0 = 0;
+        for (int s = 0; s < n_in && rc == TNLM_OK; ++s) {
+            const int z1 = s == n_in - 1 ? p->nz : std::min(p->nz, zin[s + 1] + look);
+            if (z1 > z0) {
+                const size_t off = (size_t)z0 * plane;
+                ck(cudaMemcpy2DAsync(g_dev + off, pitch, g_host + off, pitch, (size_t)(z1 - z0) * plane * sizeof(float),
+                                     (size_t)p->n_phase, cudaMemcpyHostToDevice, cs), "H2D chunk");
+                z0 = z1;
+            }
             ck(cudaEventRecord(ev_in[s], cs), "event record");
         }
     }
@@ -306,15 +340,10 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
         if (!first && !last) {
             rc = launch_sweep(p, cur, g_dev, cur, dst, 0, p->nz, kws, kws_bytes, st, variant);
         } else {
-            for (int s = 0; s < NS && rc == TNLM_OK; ++s) {
-                // slab s of the first sweep reads planes up to the end of its last z-tile plus the halo: wait for the
-                // slab that holds the last of them (the copy stream delivers the slabs in order)
-                if (first) {
-                    const int last_plane = std::min(p->nz - 1, zb[s + 1] - 1 + (kMaxRZ - 1) + halo);
-                    int need = s;
-                    while (need + 1 < NS && zb[need + 1] <= last_plane) ++need;
-                    ck(cudaStreamWaitEvent(st, ev_in[need], 0), "stream wait");
-                }
+            const std::vector<int> &zb = first ? zin : zout;
+            const int ns = (int)zb.size() - 1;
+            for (int s = 0; s < ns && rc == TNLM_OK; ++s) {
+                if (first) ck(cudaStreamWaitEvent(st, ev_in[s], 0), "stream wait");
                 if (rc == TNLM_OK) rc = launch_sweep(p, cur, g_dev, cur, dst, zb[s], zb[s + 1], kws, kws_bytes, st, variant);
                 if (last && rc == TNLM_OK) {
                     const size_t off = (size_t)zb[s] * plane;
@@ -332,10 +361,8 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
     // drain both streams whatever happened, then release the internal objects
     cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(cs);
     if (rc == TNLM_OK) { ck(e1, "enhance_host sync"); ck(e2, "enhance_host copy sync"); }
-    for (int s = 0; s < NS; ++s) {
-        if (ev_in[s]) cudaEventDestroy(ev_in[s]);
-        if (ev_out[s]) cudaEventDestroy(ev_out[s]);
-    }
+    for (cudaEvent_t ev : ev_in) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : ev_out) if (ev) cudaEventDestroy(ev);
     if (ev_start) cudaEventDestroy(ev_start);
     cudaStreamDestroy(cs);
     return rc;
@@ -355,8 +382,7 @@ int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_
     float *fi_dev = (float *)((char *)dev_ws + sba);
     float *fo_dev = (float *)((char *)dev_ws + 2 * sba);
     void *ws = (char *)dev_ws + 3 * sba;
-    const int halo = p->search_radius + p->patch_radius;
-    if (!f_init_host && n_iter >= 1 && p->nz >= 32 && p->nz / 4 / 8 * 8 >= halo + 8)
+    if (!f_init_host && n_iter >= 1 && p->nz >= 32)
         return enhance_host_pipelined(p, g_host, f_out_host, n_iter, g_dev, fo_dev, ws, dev_ws_bytes - 3 * sba, st,
                                       pick_variant(p, TNLM_VARIANT_AUTO));
     cudaError_t e = cudaMemcpyAsync(g_dev, g_host, sb, cudaMemcpyHostToDevice, st);

@@ -314,7 +314,8 @@ def test_enhance_host_matches_device_path(T):
     assert torch.equal(out_h, out_d.cpu())
 
 
-@pytest.mark.parametrize("nz,n_iter,M,d", [(40, 1, 2, 1), (37, 2, 2, 1), (64, 3, 1, 1), (48, 2, 3, 1), (44, 2, 1, 2)])
+@pytest.mark.parametrize("nz,n_iter,M,d", [(40, 1, 2, 1), (37, 2, 2, 1), (64, 3, 1, 1), (48, 2, 3, 1), (44, 2, 1, 2),
+                                            (32, 2, 4, 2), (130, 2, 2, 1), (121, 1, 2, 1)])
 def test_enhance_host_pipelined_slabs_bitwise(T, nz, n_iter, M, d):
     """Volumes of 32+ planes take the pipelined host path (slab-wise H2D / first sweep, last sweep / D2H on a second
     stream): same bits as the device path, pinned or pageable host memory, and the call may be repeated."""
