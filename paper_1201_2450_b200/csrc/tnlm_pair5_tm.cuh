@@ -11,6 +11,9 @@
 //     offsets first (its planes [M, M+RZ+4) are in the initial fill), then tz ascending; the slot of a dead plane is
 //     refilled with cp.async M+1 pass groups before its first use.
 // 168 registers and 73 KB per CTA at M = 2 (three CTAs per SM; tnlm_pair5_kernel: 252 registers, 110 KB, two).
+// At three CTAs per SM the 5-tap z-sums of the four output planes also share their pair sums (9 additions instead of
+// 16, ZSHARE below: 0.411 -> 0.426 of the FP32 roofline at the 5^3 window); in the two-CTA kernels of the 7^3 / 9^3
+// windows the same form costs the pass its register allocation (0.415 -> 0.354), so they keep the four-plane ring.
 // The order of the passes differs from tnlm_pair5_kernel's, so the two agree to rounding, not bit for bit.
 #pragma once
 #include "tnlm_pair5.cuh"
@@ -40,13 +43,15 @@ template <int M, int RZ> struct Pair5TmGeom {
 __device__ __forceinline__ unsigned tm_at(const int c, const unsigned t1, const unsigned t2) { return c < 128 ? t1 + c : t2 + (c - 128); }
 
 // One pass: W consecutive x-offsets at fixed (ty, tz), marching the RZ+4 planes (pair5_pass with TMEM operands and ring slots).
-template <typename G, int RZ, int W, bool CAREFUL>
+// ZSHARE: the z-sums of the four output planes share their pair sums (below); otherwise a four-plane ring.
+template <typename G, int RZ, int W, bool CAREFUL, bool ZSHARE>
 __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsigned t2, const float2 *__restrict__ bRow,
                                                   const float c2, const unsigned mask, const int s0)
 {
     constexpr int NVB = (W + 6) / 2, B_PLANE = G::NPB * G::PB2, NR = G::NR;
+    static_assert(!ZSHARE || RZ == 4, "the shared z-sums below are written out for four output planes");
     const float2 nc2 = make_float2(-c2, -c2);
-    float2 ring[4][W][2];
+    float2 zr[4][W][2];   // z-sum state: the last four planes' X (ring), or see a2z below (ZSHARE)
     float2 cand1[W + 1], cand2[W + 1];
     unsigned fail = 0u;
     float a8[2][8], a4[2][4], zn[2][8], bt[2][4];   // double-buffered TMEM loads
@@ -94,8 +99,25 @@ __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsig
                 float2 D[W];
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    const float2 S = add2(add2(add2(ring[0][q][i], ring[1][q][i]), add2(ring[2][q][i], ring[3][q][i])),
-                                          X[q][i]);                                       // a2z
+                    // a2z: S_o = X_o + .. + X_o+4 with the pair sums P_k = X_k + X_k+1 shared between outputs:
+                    // S_0 = X_0 + (P_1 + P_3), S_1 = (P_1 + P_3) + X_5, S_2 = X_2 + (P_3 + P_5), S_3 = (P_3 + P_5) + X_7
+                    // (9 additions for 4 outputs instead of 16; direct sums, no differences)
+                    float2 S;
+                    if (!ZSHARE) {
+                        S = add2(add2(add2(zr[0][q][i], zr[1][q][i]), add2(zr[2][q][i], zr[3][q][i])), X[q][i]);
+                    } else if (p == 4) {
+                        zr[3][q][i] = add2(zr[3][q][i], X[q][i]);                         // P_3
+                        zr[1][q][i] = add2(zr[1][q][i], zr[3][q][i]);                     // P_1 + P_3
+                        S = add2(zr[0][q][i], zr[1][q][i]);
+                    } else if (p == 5) {
+                        S = add2(zr[1][q][i], X[q][i]);
+                    } else if (p == 6) {
+                        zr[0][q][i] = add2(zr[0][q][i], X[q][i]);                         // P_5 (zr[0] held X_5)
+                        zr[3][q][i] = add2(zr[3][q][i], zr[0][q][i]);                     // P_3 + P_5
+                        S = add2(zr[2][q][i], zr[3][q][i]);
+                    } else {
+                        S = add2(zr[3][q][i], X[q][i]);
+                    }
                     const float u0 = __shfl_up_sync(0xffffffffu, S.x, 1);                 // row 2l-2
                     const float u1 = __shfl_up_sync(0xffffffffu, S.y, 1);                 // row 2l-1
                     const float d0 = __shfl_down_sync(0xffffffffu, S.x, 1);               // row 2l+2
@@ -149,10 +171,20 @@ __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsig
         for (int q = 0; q < W; ++q)
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
-                ring[0][q][i] = ring[1][q][i];
-                ring[1][q][i] = ring[2][q][i];
-                ring[2][q][i] = ring[3][q][i];
-                ring[3][q][i] = X[q][i];
+                if (!ZSHARE) {
+                    zr[0][q][i] = zr[1][q][i];
+                    zr[1][q][i] = zr[2][q][i];
+                    zr[2][q][i] = zr[3][q][i];
+                    zr[3][q][i] = X[q][i];
+                    continue;
+                }
+                if (p == 0 || p == 5) zr[0][q][i] = X[q][i];                              // X_0; X_5
+                if (p == 1) zr[1][q][i] = X[q][i];                                        // X_1
+                if (p == 2) {
+                    zr[1][q][i] = add2(zr[1][q][i], X[q][i]);                             // P_1
+                    zr[2][q][i] = X[q][i];                                                // X_2
+                }
+                if (p == 3) zr[3][q][i] = X[q][i];                                        // X_3
             }
         // output x-index i, offset q reads the candidate at window element i + 2 + q of the plane two back
 #pragma unroll
@@ -257,8 +289,8 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
             auto run_chunk = [&](auto wtag, const float2 *row, const bool first) {
                 constexpr int W = decltype(wtag)::value;
                 unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
-                if (!first) fail = pair5_pass_tm<G, RZ, W, false>(t1, t2, row, dm.c2, 0u, s0);
-                if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true>(t1, t2, row, dm.c2, fail, s0);
+                if (!first) fail = pair5_pass_tm<G, RZ, W, false, NCTA == 3>(t1, t2, row, dm.c2, 0u, s0);
+                if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true, NCTA == 3>(t1, t2, row, dm.c2, fail, s0);
             };
             // the chunk holding the zero x-offset (q = M) goes first, so that the first careful pass sets the reference
             // exponents from the best candidates
