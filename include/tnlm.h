@@ -141,6 +141,15 @@ int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_
                       int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream);
 
 /*
+ * tnlm_enhance_host with a caller-owned copy stream for the pipelined copies (a cudaStream_t other than
+ * `cuda_stream`, on the same device; NULL = the call creates and destroys one, as tnlm_enhance_host does).  The copy
+ * stream is ordered after the work already queued on `cuda_stream`, and both streams are synchronised before the
+ * call returns.  A caller that enhances many stacks saves the stream creation per call.
+ */
+int tnlm_enhance_host_streams(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
+                              int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream, void *copy_stream);
+
+/*
  * Z-slab form of one sweep for data-parallel sharding: computes only the
  * output planes z in [z_begin, z_end) of every phase.  f, g, ref and f_out are FULL stacks (the rank
  * needs planes within M+d of its slab to be valid in f / ref); planes outside the slab are untouched.

@@ -16,7 +16,7 @@ VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED, VARIANT_PAIRED_TME
 # every symbol include/tnlm.h declares
 EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_jacobi_step",
            "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
-           "tnlm_enhance_host", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
+           "tnlm_enhance_host", "tnlm_enhance_host_streams", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
            "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_z_tile", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
            "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr",
            "tnlmr_workspace_bytes", "tnlmr_project", "tnlmr_backproject", "tnlmr_cgls", "tnlmr_reconstruct"]
@@ -70,6 +70,7 @@ def lib():
         L.tnlm_enhance.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp]
         L.tnlm_enhance_variant.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp, C.c_int]
         L.tnlm_enhance_host.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp]
+        L.tnlm_enhance_host_streams.argtypes = [pp, vp, vp, vp, i32, vp, sz, vp, vp]
         L.tnlm_strerror.argtypes = [C.c_int]; L.tnlm_strerror.restype = C.c_char_p
         L.tnlm_kernel_name.argtypes = [pp]; L.tnlm_kernel_name.restype = C.c_char_p
         L.tnlm_launches_per_sweep.argtypes = [pp]; L.tnlm_launches_per_sweep.restype = i32
@@ -331,8 +332,10 @@ def tnlm_enhance(p: TnlmParams, g, n_iter, f_init=None, f_out=None, ws=None, str
     return f_out
 
 
-def tnlm_enhance_host(p: TnlmParams, g_host, n_iter, f_out_host=None, f_init_host=None, dev_ws=None, stream=None):
-    """End-to-end form with HOST tensors (pinned for asynchronous copies); returns the host result."""
+def tnlm_enhance_host(p: TnlmParams, g_host, n_iter, f_out_host=None, f_init_host=None, dev_ws=None, stream=None,
+                      copy_stream=None):
+    """End-to-end form with HOST tensors (pinned for asynchronous copies); returns the host result.
+    copy_stream: a torch.cuda.Stream for the pipelined copies (default: the library makes one per call)."""
     import torch
     for name, t in (("g_host", g_host), ("f_init_host", f_init_host), ("f_out_host", f_out_host)):
         if t is not None and (t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous()
@@ -342,11 +345,11 @@ def tnlm_enhance_host(p: TnlmParams, g_host, n_iter, f_out_host=None, f_init_hos
         f_out_host = torch.empty(p.shape, dtype=torch.float32, pin_memory=True)
     with _Call(stream, dev_ws) as c:
         dev_ws = c.workspace(dev_ws, host_workspace_bytes(p))
-        _check(lib().tnlm_enhance_host(C.byref(p), g_host.data_ptr(),
-                                       None if f_init_host is None else f_init_host.data_ptr(),
-                                       f_out_host.data_ptr(), int(n_iter), dev_ws.data_ptr(), dev_ws.numel(),
-                                       c.handle),
-               "tnlm_enhance_host")                    # synchronises the stream before returning
+        _check(lib().tnlm_enhance_host_streams(C.byref(p), g_host.data_ptr(),
+                                               None if f_init_host is None else f_init_host.data_ptr(),
+                                               f_out_host.data_ptr(), int(n_iter), dev_ws.data_ptr(), dev_ws.numel(),
+                                               c.handle, None if copy_stream is None else copy_stream.cuda_stream),
+               "tnlm_enhance_host")                    # synchronises both streams before returning
     return f_out_host
 
 

@@ -292,7 +292,8 @@ static std::vector<int> slab_bounds(const int nz, const bool grow, const bool sh
 // are bit-identical to whole-volume sweeps (z-tiles are aligned to absolute plane indices), so the result equals
 // tnlm_enhance's bit for bit.
 static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, float *f_out_host, int32_t n_iter,
-                                  float *g_dev, float *fo_dev, void *ws, size_t ws_bytes, cudaStream_t st, int variant)
+                                  float *g_dev, float *fo_dev, void *ws, size_t ws_bytes, cudaStream_t st, int variant,
+                                  cudaStream_t caller_cs)
 {
     // planes past its end that a slab's sweep reads: the halo, and the rest of a z-tile that straddles the bound
     // (bounds are multiples of 8; the deepest tile of any sweep kernel is 8 planes)
@@ -302,11 +303,13 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
     const std::vector<int> zin = slab_bounds(p->nz, true, n_iter == 1);
     const std::vector<int> zout = n_iter == 1 ? zin : slab_bounds(p->nz, false, true);
     const int n_in = (int)zin.size() - 1, n_out = (int)zout.size() - 1;
-    cudaStream_t cs = nullptr;
+    cudaStream_t cs = caller_cs;
     std::vector<cudaEvent_t> ev_in(n_in, nullptr), ev_out(n_out, nullptr);
     cudaEvent_t ev_start = nullptr;
-    cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return cuda_fail(e, "copy stream");
+    if (!caller_cs) {
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return cuda_fail(e, "copy stream");
+    }
     int rc = TNLM_OK;
     auto fail = [&](cudaError_t err, const char *what) { rc = cuda_fail(err, what); };
     auto ck = [&](cudaError_t err, const char *what) { if (err != cudaSuccess && rc == TNLM_OK) fail(err, what); return err == cudaSuccess; };
@@ -364,12 +367,18 @@ static int enhance_host_pipelined(const tnlm_params *p, const float *g_host, flo
     for (cudaEvent_t ev : ev_in) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : ev_out) if (ev) cudaEventDestroy(ev);
     if (ev_start) cudaEventDestroy(ev_start);
-    cudaStreamDestroy(cs);
+    if (!caller_cs) cudaStreamDestroy(cs);
     return rc;
 }
 
 int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
                       int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream)
+{
+    return tnlm_enhance_host_streams(p, g_host, f_init_host, f_out_host, n_iter, dev_ws, dev_ws_bytes, cuda_stream, nullptr);
+}
+
+int tnlm_enhance_host_streams(const tnlm_params *p, const float *g_host, const float *f_init_host, float *f_out_host,
+                              int32_t n_iter, void *dev_ws, size_t dev_ws_bytes, void *cuda_stream, void *copy_stream)
 {
     int rc = check_params(p);
     if (rc) return rc;
@@ -384,7 +393,7 @@ int tnlm_enhance_host(const tnlm_params *p, const float *g_host, const float *f_
     void *ws = (char *)dev_ws + 3 * sba;
     if (!f_init_host && n_iter >= 1 && p->nz >= 32)
         return enhance_host_pipelined(p, g_host, f_out_host, n_iter, g_dev, fo_dev, ws, dev_ws_bytes - 3 * sba, st,
-                                      pick_variant(p, TNLM_VARIANT_AUTO));
+                                      pick_variant(p, TNLM_VARIANT_AUTO), (cudaStream_t)copy_stream);
     cudaError_t e = cudaMemcpyAsync(g_dev, g_host, sb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(e, "H2D g");
     if (f_init_host) {

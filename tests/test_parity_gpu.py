@@ -328,6 +328,7 @@ def test_enhance_host_pipelined_slabs_bitwise(T, nz, n_iter, M, d):
     for _ in range(2):
         assert torch.equal(T.tnlm_enhance_host(p, gh, n_iter), want)
     assert torch.equal(T.tnlm_enhance_host(p, torch.from_numpy(g), n_iter, f_out_host=torch.empty(shape)), want)
+    assert torch.equal(T.tnlm_enhance_host(p, gh, n_iter, copy_stream=torch.cuda.Stream()), want)   # caller-owned copy stream
 
 
 def test_device_error_codes(T):
