@@ -56,7 +56,8 @@ typedef enum {
     TNLM_ERR_ALIAS = -5,        /* f_out overlaps an input (Jacobi reads only the old iterate,
                                    PAPER.md:176) or the workspace                                  */
     TNLM_ERR_WORKSPACE = -6,    /* workspace NULL, too small or not 16-byte aligned                */
-    TNLM_ERR_CUDA = -7          /* a CUDA call failed; tnlm_strerror(TNLM_ERR_CUDA) has the text   */
+    TNLM_ERR_CUDA = -7,         /* a CUDA call failed; tnlm_strerror(TNLM_ERR_CUDA) has the text   */
+    TNLM_ERR_TOO_LARGE = -8     /* larger than the fixed scratch of a *_static entry point         */
 } tnlm_status;
 
 /* Kernel variants, for tests and benchmarks.  AUTO picks the fastest one compiled for (d, M):
@@ -183,6 +184,23 @@ int tnlm_srr(const tnlm_params *p, const float *f_fdk, const float *f_enh, const
              void *ws, size_t ws_bytes, void *cuda_stream);
 int tnlm_cnr(const tnlm_params *p, const float *stack, int32_t phase, const int32_t *roi, const int32_t *roi_bg,
              double *out5, void *cuda_stream);
+
+/*
+ * tnlm_srr for callers that must not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same result as tnlm_srr (Eq. 10), no `ws` argument.  The two
+ * per-phase TV sums live in a static device array inside the library of 2 * TNLM_SRR_STATIC_MAX_PHASES doubles
+ * (1 KB, held by every GPU that loads the library until the process exits); the call itself allocates nothing (no
+ * cudaMalloc / cudaFree, no allocating library routine; the first call on a device looks the array's address up once).
+ * n_phase > TNLM_SRR_STATIC_MAX_PHASES is refused with TNLM_ERR_TOO_LARGE: use tnlm_srr with a caller workspace.
+ * Inputs and srr_out (n_phase doubles, DEVICE, 8-byte aligned) are the caller's, as in tnlm_srr.  Every call on a
+ * device shares the one array: the call clears the sums it uses on `cuda_stream` before accumulating, so calls
+ * queued on ONE stream are safe back to back, but two calls that can overlap on the GPU (different streams, or
+ * different host threads on different streams) RACE on it and give wrong ratios -- serialise them, or use tnlm_srr.
+ * Other errors as tnlm_srr.
+ */
+#define TNLM_SRR_STATIC_MAX_PHASES 64
+int tnlm_srr_static(const tnlm_params *p, const float *f_fdk, const float *f_enh, const float *f_star,
+                    double *srr_out, void *cuda_stream);
 
 /* Message for a status code; for TNLM_ERR_CUDA includes the calling thread's last CUDA error text. */
 const char *tnlm_strerror(int code);

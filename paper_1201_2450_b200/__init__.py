@@ -7,12 +7,12 @@ compute call requires the compiled library and CUDA tensors and fails loudly oth
 """
 from .binding import (TnlmParams, TnlmError, lib, library_path, workspace_bytes, weights_bytes,
                       host_workspace_bytes, tnlm_weights, tnlm_jacobi_step, tnlm_enhance, tnlm_enhance_host,
-                      tnlm_jacobi_step_slab, tnlm_tv_diff, tnlm_srr, tnlm_cnr, kernel_name, launches_per_sweep, z_tile, probe_fp32, strerror,
+                      tnlm_jacobi_step_slab, tnlm_tv_diff, tnlm_srr, tnlm_srr_static, tnlm_cnr, kernel_name, launches_per_sweep, z_tile, probe_fp32, strerror,
                       VARIANT_AUTO, VARIANT_GENERIC, VARIANT_TILED, VARIANT_PAIRED, VARIANT_PAIRED_TMEM, EXPORTS,
                       TnlmrGeometry, tnlmr_workspace_bytes, tnlmr_project, tnlmr_backproject, tnlmr_cgls, tnlmr_reconstruct)
 
 __all__ = ["TnlmParams", "TnlmError", "lib", "library_path", "workspace_bytes", "weights_bytes",
            "host_workspace_bytes", "tnlm_weights", "tnlm_jacobi_step", "tnlm_enhance", "tnlm_enhance_host",
-           "tnlm_jacobi_step_slab", "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr", "kernel_name", "launches_per_sweep", "z_tile", "probe_fp32", "strerror",
+           "tnlm_jacobi_step_slab", "tnlm_tv_diff", "tnlm_srr", "tnlm_srr_static", "tnlm_cnr", "kernel_name", "launches_per_sweep", "z_tile", "probe_fp32", "strerror",
            "VARIANT_AUTO", "VARIANT_GENERIC", "VARIANT_TILED", "VARIANT_PAIRED", "VARIANT_PAIRED_TMEM", "EXPORTS",
            "TnlmrGeometry", "tnlmr_workspace_bytes", "tnlmr_project", "tnlmr_backproject", "tnlmr_cgls", "tnlmr_reconstruct"]

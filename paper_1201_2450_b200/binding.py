@@ -18,7 +18,7 @@ EXPORTS = ["tnlm_workspace_bytes", "tnlm_weights_bytes", "tnlm_weights", "tnlm_j
            "tnlm_jacobi_step_variant", "tnlm_enhance", "tnlm_enhance_variant", "tnlm_host_workspace_bytes",
            "tnlm_enhance_host", "tnlm_enhance_host_streams", "tnlm_jacobi_step_slab", "tnlm_jacobi_step_slab_variant", "tnlm_strerror",
            "tnlm_kernel_name", "tnlm_launches_per_sweep", "tnlm_z_tile", "tnlm_probe_fp32", "tnlm_probe_fp32_ffma_count",
-           "tnlm_tv_diff", "tnlm_srr", "tnlm_cnr",
+           "tnlm_tv_diff", "tnlm_srr", "tnlm_srr_static", "tnlm_cnr",
            "tnlmr_workspace_bytes", "tnlmr_project", "tnlmr_backproject", "tnlmr_cgls", "tnlmr_reconstruct"]
 
 
@@ -83,6 +83,7 @@ def lib():
         L.tnlmr_reconstruct.argtypes = [gp, pp, vp, vp, vp, vp, i32, i32, i32, vp, C.c_size_t, vp]; L.tnlmr_reconstruct.restype = C.c_int
         L.tnlm_tv_diff.argtypes = [pp, vp, vp, vp, vp]
         L.tnlm_srr.argtypes = [pp, vp, vp, vp, vp, vp, sz, vp]
+        L.tnlm_srr_static.argtypes = [pp, vp, vp, vp, vp, vp]
         L.tnlm_cnr.argtypes = [pp, vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), vp, vp]
         L.tnlm_probe_fp32.argtypes = [i32, vp, vp]
         L.tnlm_probe_fp32_ffma_count.argtypes = [i32]; L.tnlm_probe_fp32_ffma_count.restype = C.c_double
@@ -379,6 +380,24 @@ def tnlm_srr(p: TnlmParams, f_fdk, f_enh, f_star, stream=None):
         _check(lib().tnlm_srr(C.byref(p), _dev_ptr(f_fdk, p, "f_fdk"), _dev_ptr(f_enh, p, "f_enh"),
                               _dev_ptr(f_star, p, "f_star"), out.data_ptr(), ws.data_ptr(), ws.numel() * 8,
                               c.handle), "tnlm_srr")
+    return out
+
+
+SRR_STATIC_MAX_PHASES = 64   # TNLM_SRR_STATIC_MAX_PHASES of include/tnlm.h
+
+
+def tnlm_srr_static(p: TnlmParams, f_fdk, f_enh, f_star, out=None, stream=None):
+    """tnlm_srr without a workspace: the library keeps the scratch in a static device array (n_phase <= 64), so
+    the C call allocates nothing.  Pass `out` (float64 CUDA tensor [n_phase]) to keep this wrapper allocation-free
+    too.  Calls that overlap on the GPU race on the shared scratch (include/tnlm.h)."""
+    import torch
+    with _Call(stream, f_fdk, f_enh, f_star, out) as c:
+        if out is None:
+            out = torch.empty(p.n_phase, dtype=torch.float64, device=c.device)
+        elif not out.is_cuda or out.dtype != torch.float64 or not out.is_contiguous() or out.numel() != p.n_phase:
+            raise TypeError(f"out must be a contiguous float64 CUDA tensor of {p.n_phase} elements")
+        _check(lib().tnlm_srr_static(C.byref(p), _dev_ptr(f_fdk, p, "f_fdk"), _dev_ptr(f_enh, p, "f_enh"),
+                                     _dev_ptr(f_star, p, "f_star"), out.data_ptr(), c.handle), "tnlm_srr_static")
     return out
 
 

@@ -448,6 +448,65 @@ int tnlm_srr(const tnlm_params *p, const float *f_fdk, const float *f_enh, const
     return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "srr launch");
 }
 
+// ---- tnlm_srr for callers that cannot allocate (tnlm.h: tnlm_srr_static) -----------------------------------------
+// The two per-phase TV sums that tnlm_srr keeps in the caller's `ws` live in a file-scope device array: 2 x
+// TNLM_SRR_STATIC_MAX_PHASES doubles (1 KB) that every GPU which loads the library holds until the process exits.
+// In host code `g_srr_scratch` is only a stand-in for the symbol, not a device address; the address of the current
+// device's copy comes from cudaGetSymbolAddress, looked up once per device and cached.
+}  // extern "C"
+
+namespace {
+
+static __device__ __align__(256) double g_srr_scratch[2 * TNLM_SRR_STATIC_MAX_PHASES];
+
+constexpr int kSrrMaxDevices = 64;
+std::atomic<double *> g_srr_scratch_addr[kSrrMaxDevices];   // per device ordinal, nullptr until looked up
+
+// Device address of the current device's g_srr_scratch.  Two threads that race on the first call of a device both
+// look the address up and store the same value.
+int srr_scratch_ptr(double **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "srr_static: cudaGetDevice");
+    if (dev < 0 || dev >= kSrrMaxDevices) return cuda_fail(cudaErrorInvalidDevice, "srr_static: device ordinal beyond the address table");
+    double *ptr = g_srr_scratch_addr[dev].load(std::memory_order_acquire);
+    if (!ptr) {
+        e = cudaGetSymbolAddress((void **)&ptr, g_srr_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "srr_static: cudaGetSymbolAddress");
+        if (!ptr) return cuda_fail(cudaErrorInvalidSymbol, "srr_static: cudaGetSymbolAddress returned NULL");
+        g_srr_scratch_addr[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return TNLM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tnlm_srr_static(const tnlm_params *p, const float *f_fdk, const float *f_enh, const float *f_star, double *srr_out,
+                    void *cuda_stream)
+{
+    int rc = check_params(p);
+    if (rc) return rc;
+    if (!f_fdk || !f_enh || !f_star || !srr_out) return TNLM_ERR_NULL_POINTER;
+    if (p->n_phase > TNLM_SRR_STATIC_MAX_PHASES) return TNLM_ERR_TOO_LARGE;
+    if ((uintptr_t)srr_out & 7u) return TNLM_ERR_WORKSPACE;
+    double *t = nullptr;
+    rc = srr_scratch_ptr(&t);
+    if (rc) return rc;
+    // the array keeps the previous call's sums: tnlm_tv_diff clears its n_phase outputs on the stream before it
+    // accumulates into them, so each half starts at zero
+    rc = tnlm_tv_diff(p, f_fdk, f_star, t, cuda_stream);
+    if (rc) return rc;
+    rc = tnlm_tv_diff(p, f_enh, f_star, t + p->n_phase, cuda_stream);
+    if (rc) return rc;
+    srr_finish_kernel<<<(p->n_phase + 63) / 64, 64, 0, (cudaStream_t)cuda_stream>>>(t, srr_out, p->n_phase);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? TNLM_OK : cuda_fail(e, "srr_static launch");
+}
+
 int tnlm_cnr(const tnlm_params *p, const float *stack, int32_t phase, const int32_t *roi, const int32_t *roi_bg,
              double *out5, void *cuda_stream)
 {
@@ -495,6 +554,7 @@ const char *tnlm_strerror(int code)
         case TNLM_ERR_ALIAS: return "output overlaps an input or the workspace";
         case TNLM_ERR_WORKSPACE: return "workspace or stack pointer NULL, too small or not 16-byte aligned";
         case TNLM_ERR_CUDA: return g_cuda_err;
+        case TNLM_ERR_TOO_LARGE: return "problem larger than the fixed scratch of a *_static entry point (tnlm_srr_static: n_phase > TNLM_SRR_STATIC_MAX_PHASES)";
         default: return "unknown tnlm status";
     }
 }

@@ -94,7 +94,12 @@ def test_argument_errors_are_synchronous(T):
     assert L.tnlm_weights(C.byref(p), None, D, None, 0, None) == -1
     assert L.tnlm_enhance_host(C.byref(p), A, None, D, 1, W, 16, None) == -6
     assert L.tnlm_probe_fp32(1, None, None) == -1
-    for code in range(0, -8, -1):
+    # tnlm_srr_static: argument errors come before any CUDA call, the phase limit has its own code
+    big = T.TnlmParams.make((65, 2, 4, 4), 1, 1, 0.1, 1.0)
+    assert L.tnlm_srr_static(C.byref(big), A, B, A, D, None) == -8
+    assert L.tnlm_srr_static(C.byref(p), A, B, None, D, None) == -1
+    assert L.tnlm_srr_static(C.byref(p), A, B, A, D + 4, None) == -6
+    for code in range(0, -9, -1):
         assert T.strerror(code) not in ("", "unknown tnlm status")
 
 
