@@ -11,6 +11,7 @@
 //     offsets first (its planes [M, M+RZ+4) are in the initial fill), then tz ascending; the slot of a dead plane is
 //     refilled with cp.async M+1 pass groups before its first use.
 // 168 registers and 73 KB per CTA at M = 2 (three CTAs per SM; tnlm_pair5_kernel: 252 registers, 110 KB, two).
+// At M = 3 (two CTAs per SM) the tile is 6 planes deep: 120 + 96 = 216 columns per thread as 128 + 128.
 // At three CTAs per SM the 5-tap z-sums of the four output planes also share their pair sums (9 additions instead of
 // 16, ZSHARE below: 0.411 -> 0.426 of the FP32 roofline at the 5^3 window); in the two-CTA kernels of the 7^3 / 9^3
 // windows the same form costs the pass its register allocation (0.415 -> 0.354), so they keep the four-plane ring.
@@ -34,8 +35,8 @@ template <int M, int RZ> struct Pair5TmGeom {
     static constexpr size_t BYTES = (size_t)R_F2 * sizeof(float2) + 16;
     // TMEM columns of a thread: a-planes (12 words each), then 16-word accumulator blocks Z[2] N[2] b[2] pad
     static constexpr int TM_A = 0, TM_ACC = (12 * NAP + 15) / 16 * 16, TM_END = TM_ACC + 16 * RZ;
-    static constexpr int TM_COLS2 = TM_END > 128 ? (TM_END > 160 ? 64 : 32) : 0;
-    static_assert(TM_END <= 128 + TM_COLS2 && TM_END <= 192, "thread-private operands do not fit the CTA's TMEM columns");
+    static constexpr int TM_COLS2 = TM_END > 128 ? (TM_END > 160 ? (TM_END > 192 ? 128 : 64) : 32) : 0;
+    static_assert(TM_END <= 128 + TM_COLS2 && TM_END <= 256, "thread-private operands do not fit the CTA's TMEM columns");
     static_assert(12 * NAP <= 128 && (TM_ACC >= 128 || (128 - TM_ACC) % 16 == 0), "a block would straddle the two allocations");
 };
 
@@ -226,6 +227,7 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(sa) : "memory");
         if (G::TM_COLS2 == 32) asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" :: "r"(sa + 4) : "memory");
         if (G::TM_COLS2 == 64) asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" :: "r"(sa + 4) : "memory");
+        if (G::TM_COLS2 == 128) asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(sa + 4) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -369,6 +371,7 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tm_base1) : "memory");
         if (G::TM_COLS2 == 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 32;" :: "r"(tm_base2) : "memory");
         if (G::TM_COLS2 == 64) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" :: "r"(tm_base2) : "memory");
+        if (G::TM_COLS2 == 128) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tm_base2) : "memory");
     }
 }
 
@@ -393,7 +396,11 @@ cudaError_t launch_pair5_tmr_t(const Dims &dm, const float *f, const float *g, f
 // ---------------------------------------------------------------------------------------------
 // TNLM_VARIANT_PAIRED_TMEM (ref == f): 3^3 patch: whole tile resident at M = 2 (tnlm_pair_tm_kernel), rolling window at
 // M = 3, 4 (tnlm_pair_tmr_kernel); 5^3 patch: rolling window at M = 2, 3, 4 (tnlm_pair5_tmr_kernel).  The 3^3 windows
-// stay on tnlm_pair_kernel / tnlm_pair5_kernel (measured: no gain there).
+// stay on tnlm_pair_kernel / tnlm_pair5_kernel (measured: no gain there).  Where two CTAs per SM are all that fits anyway
+// (3^3 patch at M = 4, 5^3 patch at M = 3) the z-tile is 6 planes deep: a CTA may then take 256 TMEM columns, and the
+// z-halo of the march drops from 6/4 to 8/6 (5^3 patch: 8/4 to 10/6).  +3.6 % and +6.4 % at 128 planes (which 6 does not
+// divide), +4.6 % and +9.7 % at 120.  At M = 4 the 5^3-patch ring does not fit twice at RZ = 6; the three-CTA shapes lose
+// more from the third CTA than the deeper tile gives back (measured, profiles/r02_config5_sweep.md).
 inline bool pair_tm_supported(const tnlm_params &p)
 {
     return (p.patch_radius == 1 || p.patch_radius == 2) && p.search_radius >= 2 && p.search_radius <= 4;
@@ -421,7 +428,7 @@ inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const fl
     if (p.patch_radius == 2) {
         switch (p.search_radius) {
             case 2: return launch_pair5_tmr_t<2, 4, 3>(dm, f, g, f_out, st);           // <M, RZ, CTAs per SM>
-            case 3: return launch_pair5_tmr_t<3, 4, 2>(dm, f, g, f_out, st);
+            case 3: return launch_pair5_tmr_t<3, 6, 2>(dm, f, g, f_out, st);           // deep tile: 128 + 128 TMEM columns
             case 4: return launch_pair5_tmr_t<4, 4, 2>(dm, f, g, f_out, st);
             default: return cudaErrorNotSupported;
         }
@@ -429,7 +436,7 @@ inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const fl
     switch (p.search_radius) {
         case 2: return launch_pair_tm_t<2, 4, 16, 3, true>(dm, f, g, f_out, st);   // <M, RZ, TX, CTAs per SM, b in TMEM>
         case 3: return launch_pair_tmr_t<3, 4, 3>(dm, f, g, f_out, st);            // <M, RZ, CTAs per SM>
-        case 4: return launch_pair_tmr_t<4, 4, 2>(dm, f, g, f_out, st);
+        case 4: return launch_pair_tmr_t<4, 6, 2>(dm, f, g, f_out, st);            // deep tile: 256 TMEM columns
         default: return cudaErrorNotSupported;
     }
 }

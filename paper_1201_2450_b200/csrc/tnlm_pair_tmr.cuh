@@ -10,6 +10,8 @@
 // it is first read.  With the -ref_i windows and (Z, N, b) in TMEM (tnlm_pair_tm.cuh) a CTA needs 69 KB at M = 3,
 // RZ = 4: three CTAs per SM, 12 warps.  Same arithmetic per pass; the ORDER of the passes differs from
 // tnlm_pair_kernel's (centre row, then tz ascending), so results agree with it to rounding, not bit for bit.
+// At M = 4 only two CTAs fit whatever the depth, so the tile is 6 planes deep there (z-halo 8/6 instead of 6/4 on a1 /
+// a2x, 160 TMEM columns per thread out of an allocation of 256): 0.548 -> 0.568 of the FP32 roofline at 128 planes.
 #pragma once
 #include "tnlm_pair_tm.cuh"
 
@@ -23,11 +25,26 @@ __device__ __forceinline__ void cp_async4(float *smem_dst, const float *gmem_src
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int M, int RZ> struct PairTmrGeom : PairTmGeom<M, RZ, 16, true> {
-    using B = PairTmGeom<M, RZ, 16, true>;
+// Tile geometry (PairTmGeom's for TX = 16 with (Z, N, b) in TMEM, plus the ring).  Deep tiles need more than 128 TMEM
+// columns per thread (RZ = 6: 64 + 96 = 160): the CTA then allocates 256, which leaves room for two CTAs per SM.
+template <int M, int RZ> struct PairTmrGeom {
+    using C = Chunks<M>;
+    static constexpr int TX = 16, NT = 128;
+    static constexpr int E = 2 * M + 1;
+    static constexpr int NVB0 = (C::W0 + 4) / 2;
+    static constexpr int NVB1 = C::W1 ? (C::W1 + 4) / 2 : 0;
+    static constexpr int BCOLS = TX + 2 * M + 2;
+    static constexpr int BREAD = cmax(TX - 2 + 2 * NVB0, C::W1 ? TX - 2 + 4 + 2 * NVB1 : 0);
+    static constexpr int PB2 = pitch2(cmax(BCOLS, BREAD));
+    static constexpr int NPE = 16 + M, NPO = 15 + M, NPB = NPE + NPO;
+    static constexpr int NAP = RZ + 2, NBP = RZ + 2 + 2 * M;
     static constexpr int NR = RZ + 2 + M;            // ring slots; the initial fill [0, NR) holds the centre window
-    static constexpr int R_F2 = NR * B::NPB * B::PB2;
-    static constexpr size_t BYTES = (size_t)R_F2 * sizeof(float2) + 16;
+    static constexpr int R_F2 = NR * NPB * PB2;
+    static constexpr size_t BYTES = (size_t)R_F2 * sizeof(float2) + 16;   // + the TMEM base-address slot
+    static constexpr int ACC_W = 16;                 // words per output plane: Z[2], N[2], b[2], 4 words of padding
+    static constexpr int TM_A = 0, TM_ACC = 8 * NAP;
+    static constexpr int TM_COLS = TM_ACC + ACC_W * RZ <= 128 ? 128 : 256;   // columns the CTA allocates
+    static_assert(TM_ACC + ACC_W * RZ <= TM_COLS, "thread-private operands do not fit the CTA's TMEM columns");
 };
 
 // Fetch plane `pz` of the clamped ref_j tile (rows y = yo + r, columns x = xo + c) into ring slot `slot`, both row-pair
