@@ -12,9 +12,8 @@
 //     refilled with cp.async M+1 pass groups before its first use.
 // 168 registers and 73 KB per CTA at M = 2 (three CTAs per SM; tnlm_pair5_kernel: 252 registers, 110 KB, two).
 // At M = 3 (two CTAs per SM) the tile is 6 planes deep: 120 + 96 = 216 columns per thread as 128 + 128.
-// At three CTAs per SM the 5-tap z-sums of the four output planes also share their pair sums (9 additions instead of
-// 16, ZSHARE below: 0.411 -> 0.426 of the FP32 roofline at the 5^3 window); in the two-CTA kernels of the 7^3 / 9^3
-// windows the same form costs the pass its register allocation (0.415 -> 0.354), so they keep the four-plane ring.
+// The 5-tap z-sums of the output planes share their pair sums (two additions per output instead of four, ZSHARE below:
+// 0.411 -> 0.427 of the FP32 roofline at the 5^3 window, 0.442 -> 0.449 at the 7^3 window).
 // The order of the passes differs from tnlm_pair5_kernel's, so the two agree to rounding, not bit for bit.
 #pragma once
 #include "tnlm_pair5.cuh"
@@ -50,9 +49,10 @@ __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsig
                                                   const float c2, const unsigned mask, const int s0)
 {
     constexpr int NVB = (W + 6) / 2, B_PLANE = G::NPB * G::PB2, NR = G::NR;
-    static_assert(!ZSHARE || RZ == 4, "the shared z-sums below are written out for four output planes");
+    static_assert(!ZSHARE || RZ % 2 == 0, "the shared z-sums pair the output planes");
     const float2 nc2 = make_float2(-c2, -c2);
-    float2 zr[4][W][2];   // z-sum state: the last four planes' X (ring), or see a2z below (ZSHARE)
+    float2 zr[4][W][2];                                    // z-sum state: the last four planes' X (ring) ...
+    float2 ze[2][W][2], zo[W][2], zp[W][2], zq[W][2];      // ... or the shared sums of ZSHARE (a2z below)
     float2 cand1[W + 1], cand2[W + 1];
     unsigned fail = 0u;
     float a8[2][8], a4[2][4], zn[2][8], bt[2][4];   // double-buffered TMEM loads
@@ -100,24 +100,20 @@ __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsig
                 float2 D[W];
 #pragma unroll
                 for (int q = 0; q < W; ++q) {
-                    // a2z: S_o = X_o + .. + X_o+4 with the pair sums P_k = X_k + X_k+1 shared between outputs:
-                    // S_0 = X_0 + (P_1 + P_3), S_1 = (P_1 + P_3) + X_5, S_2 = X_2 + (P_3 + P_5), S_3 = (P_3 + P_5) + X_7
-                    // (9 additions for 4 outputs instead of 16; direct sums, no differences)
+                    // a2z: S_o = X_o + .. + X_o+4.  ZSHARE: with the pair sums P_k = X_k + X_k+1 (k odd) and
+                    // Q_k = P_k + P_k+2 the outputs (o, o+1), o even, share Q_o+1: S_o = X_o + Q_o+1 at plane o+4,
+                    // S_o+1 = Q_o+1 + X_o+5 at plane o+5 -- two additions per output instead of four; direct sums, no
+                    // differences.  State: the even planes' X (two alive), the last odd X, the last P, the last Q.
                     float2 S;
                     if (!ZSHARE) {
                         S = add2(add2(add2(zr[0][q][i], zr[1][q][i]), add2(zr[2][q][i], zr[3][q][i])), X[q][i]);
-                    } else if (p == 4) {
-                        zr[3][q][i] = add2(zr[3][q][i], X[q][i]);                         // P_3
-                        zr[1][q][i] = add2(zr[1][q][i], zr[3][q][i]);                     // P_1 + P_3
-                        S = add2(zr[0][q][i], zr[1][q][i]);
-                    } else if (p == 5) {
-                        S = add2(zr[1][q][i], X[q][i]);
-                    } else if (p == 6) {
-                        zr[0][q][i] = add2(zr[0][q][i], X[q][i]);                         // P_5 (zr[0] held X_5)
-                        zr[3][q][i] = add2(zr[3][q][i], zr[0][q][i]);                     // P_3 + P_5
-                        S = add2(zr[2][q][i], zr[3][q][i]);
+                    } else if ((p & 1) == 0) {
+                        const float2 pn = add2(zo[q][i], X[q][i]);                        // P_p-1
+                        zq[q][i] = add2(zp[q][i], pn);                                    // Q_p-3
+                        zp[q][i] = pn;
+                        S = add2(ze[(p >> 1) & 1][q][i], zq[q][i]);                       // X_p-4 + Q_p-3
                     } else {
-                        S = add2(zr[3][q][i], X[q][i]);
+                        S = add2(zq[q][i], X[q][i]);                                      // Q_p-4 + X_p
                     }
                     const float u0 = __shfl_up_sync(0xffffffffu, S.x, 1);                 // row 2l-2
                     const float u1 = __shfl_up_sync(0xffffffffu, S.y, 1);                 // row 2l-1
@@ -179,13 +175,12 @@ __device__ __forceinline__ unsigned pair5_pass_tm(const unsigned t1, const unsig
                     zr[3][q][i] = X[q][i];
                     continue;
                 }
-                if (p == 0 || p == 5) zr[0][q][i] = X[q][i];                              // X_0; X_5
-                if (p == 1) zr[1][q][i] = X[q][i];                                        // X_1
-                if (p == 2) {
-                    zr[1][q][i] = add2(zr[1][q][i], X[q][i]);                             // P_1
-                    zr[2][q][i] = X[q][i];                                                // X_2
+                if (p & 1) {
+                    zo[q][i] = X[q][i];                                                   // the odd plane of the next P
+                } else {
+                    if (p == 2) zp[q][i] = add2(zo[q][i], X[q][i]);                       // P_1
+                    ze[(p >> 1) & 1][q][i] = X[q][i];                                     // X_p replaces X_p-4
                 }
-                if (p == 3) zr[3][q][i] = X[q][i];                                        // X_3
             }
         // output x-index i, offset q reads the candidate at window element i + 2 + q of the plane two back
 #pragma unroll
@@ -205,6 +200,7 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
 {
     using G = Pair5TmGeom<M, RZ>;
     constexpr int TX = 16, NR = G::NR, E = G::E;
+    constexpr bool kZShare = RZ % 2 == 0;   // shared z-sums (pair5_pass_tm) wherever the output planes pair up
     extern __shared__ __align__(16) float smem[];
     float2 *sBE = reinterpret_cast<float2 *>(smem);
     float2 *sBO = sBE + G::NPE * G::PB2;
@@ -291,8 +287,8 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
             auto run_chunk = [&](auto wtag, const float2 *row, const bool first) {
                 constexpr int W = decltype(wtag)::value;
                 unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
-                if (!first) fail = pair5_pass_tm<G, RZ, W, false, NCTA == 3>(t1, t2, row, dm.c2, 0u, s0);
-                if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true, NCTA == 3>(t1, t2, row, dm.c2, fail, s0);
+                if (!first) fail = pair5_pass_tm<G, RZ, W, false, kZShare>(t1, t2, row, dm.c2, 0u, s0);
+                if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true, kZShare>(t1, t2, row, dm.c2, fail, s0);
             };
             // the chunk holding the zero x-offset (q = M) goes first, so that the first careful pass sets the reference
             // exponents from the best candidates
