@@ -1,19 +1,20 @@
 // 5^3-patch sweep kernel (d = 2, ref == f) with the thread-private operands in tensor memory and a rolling ref_j window.
 //
 // tnlm_pair5_kernel's arithmetic (read tnlm_pair5.cuh first: 6 differences per 2-voxel run, 5-tap x-sums that share
-// their four middle squares, 5-tap z-sum from a four-plane register ring, 5-tap y-sum from four shuffles per row pair,
-// x-offset chunks of 2-3) with the two changes that took the 3^3-patch kernels of the 7^3 / 9^3 windows from one CTA per
-// SM to three / two (tnlm_pair_tm.cuh, tnlm_pair_tmr.cuh):
+// their four middle squares, 5-tap z-sum, 5-tap y-sum from four shuffles per row pair) with the two changes that took the
+// 3^3-patch kernels of the 7^3 / 9^3 windows from one CTA per SM to three / two (tnlm_pair_tm.cuh, tnlm_pair_tmr.cuh):
 //   * TMEM holds what only its own thread touches: the -ref_i windows (6 columns x 2 rows = 12 words per plane, RZ+4
-//     planes) and (Z, N, b) of the 4 RZ outputs (16 words per output plane).  96 + 64 = 160 columns per thread at RZ = 4:
-//     the CTA allocates 128 + 32 (three CTAs use 480 of the SM's 512).
+//     planes) and (Z, N, b) of the 4 RZ outputs (16 words per output plane).  96 + 64 = 160 columns per thread at RZ = 4
+//     (allocated as 128 + 32), 120 + 96 = 216 at RZ = 6 (128 + 128: two CTAs use all 512 columns of the SM).
 //   * shared memory holds a ring of NR = RZ+4+M planes of the doubled ref_j tile instead of all RZ+4+2M: the centre row of
 //     offsets first (its planes [M, M+RZ+4) are in the initial fill), then tz ascending; the slot of a dead plane is
 //     refilled with cp.async M+1 pass groups before its first use.
-// 168 registers and 73 KB per CTA at M = 2 (three CTAs per SM; tnlm_pair5_kernel: 252 registers, 110 KB, two).
-// At M = 3 (two CTAs per SM) the tile is 6 planes deep: 120 + 96 = 216 columns per thread as 128 + 128.
-// The 5-tap z-sums of the output planes share their pair sums (two additions per output instead of four, ZSHARE below:
-// 0.411 -> 0.427 of the FP32 roofline at the 5^3 window, 0.442 -> 0.449 at the 7^3 window).
+// and two that the room so gained pays for:
+//   * the 5-tap z-sums of the output planes share their pair sums (two additions per output instead of four, ZSHARE below);
+//   * with two CTAs per SM (~250 registers per thread instead of 168 at three) the x-offsets go in chunks of 4-5 instead
+//     of 2-3 and, where the ring fits twice (M = 2, 3), the tile is 6 planes deep.  Measured best in every shape
+//     (launch_pair_tm below); the three-CTA form <2,4,3> of the 5^3 window reaches 0.427 of the FP32 roofline, <2,6,2>
+//     0.473.
 // The order of the passes differs from tnlm_pair5_kernel's, so the two agree to rounding, not bit for bit.
 #pragma once
 #include "tnlm_pair5.cuh"
@@ -201,6 +202,8 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
     using G = Pair5TmGeom<M, RZ>;
     constexpr int TX = 16, NR = G::NR, E = G::E;
     constexpr bool kZShare = RZ % 2 == 0;   // shared z-sums (pair5_pass_tm) wherever the output planes pair up
+    constexpr bool kWide = NCTA == 2;       // two CTAs per SM have the registers for chunks of four or five x-offsets
+    constexpr bool kOneSite = kWide && M == 4;   // three chunk widths: see the pass loop
     extern __shared__ __align__(16) float smem[];
     float2 *sBE = reinterpret_cast<float2 *>(smem);
     float2 *sBO = sBE + G::NPE * G::PB2;
@@ -292,27 +295,52 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
             };
             // the chunk holding the zero x-offset (q = M) goes first, so that the first careful pass sets the reference
             // exponents from the best candidates
+            if constexpr (kWide && M == 2) {          // x-offsets 0-4
+                run_chunk(std::integral_constant<int, 5>{}, bRow, first_row);
+            } else if constexpr (kWide && M == 3) {   // x-offsets 0-3, 4-6
+                run_chunk(std::integral_constant<int, 4>{}, bRow, first_row);
+                run_chunk(std::integral_constant<int, 3>{}, bRow + 4, false);
+            } else if constexpr (kWide && M == 4) {   // x-offsets 4-5, 0-3, 6-8
+                run_chunk(std::integral_constant<int, 2>{}, bRow + 4, first_row);
+                run_chunk(std::integral_constant<int, 4>{}, bRow, false);
+                run_chunk(std::integral_constant<int, 3>{}, bRow + 6, false);
+            } else {
 #pragma unroll 1
-            for (int cc = 0; cc < M; ++cc) {
-                const int c = (cc + M / 2) % M;
-                if (c == M - 1) run_chunk(std::integral_constant<int, 3>{}, bRow + 2 * c, first_row && cc == 0);
-                else run_chunk(std::integral_constant<int, 2>{}, bRow + 2 * c, first_row && cc == 0);
+                for (int cc = 0; cc < M; ++cc) {
+                    const int c = (cc + M / 2) % M;
+                    if (c == M - 1) run_chunk(std::integral_constant<int, 3>{}, bRow + 2 * c, first_row && cc == 0);
+                    else run_chunk(std::integral_constant<int, 2>{}, bRow + 2 * c, first_row && cc == 0);
+                }
             }
         };
-        run_row(M, M, true);   // centre row first
+        auto refill = [&](const int tz) {   // before the rows of tz >= 1: plane tz - 1 is dead, plane tz - 1 + NR takes its slot
+            cp_async_wait_all();
+            __syncthreads();   // the plane fetched during the previous group is visible; every warp is done with plane tz - 1
+            const int pz = tz - 1 + NR;
+            if (pz < G::NBP)
+                stage_plane_async<G>(reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO),
+                                     fj + (size_t)clampi(Z0 - 2 - M + pz, dm.Z) * zstride, (tz - 1) % NR, Y0 - 2 - M, X0 - 2 - M, dm, tid);
+        };
+        if constexpr (kOneSite) {
+            // one call site for the rows of offsets (with three chunk widths inlined twice each the compiler would
+            // otherwise turn run_row into a function): k = -1 is the centre row, which goes first, then (tz, ty) ascending
 #pragma unroll 1
-        for (int tz = 0; tz < E; ++tz) {
-            if (tz >= 1) {
-                cp_async_wait_all();
-                __syncthreads();   // the plane fetched during the previous group is visible; every warp is done with plane tz - 1
-                const int pz = tz - 1 + NR;
-                if (pz < G::NBP)
-                    stage_plane_async<G>(reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO),
-                                         fj + (size_t)clampi(Z0 - 2 - M + pz, dm.Z) * zstride, (tz - 1) % NR, Y0 - 2 - M, X0 - 2 - M, dm, tid);
+            for (int k = -1; k < E * E; ++k) {
+                const bool centre_first = k < 0;
+                const int tz = centre_first ? M : k / E, ty = centre_first ? M : k - tz * E;
+                if (!centre_first && ty == 0 && tz >= 1) refill(tz);
+                if (!centre_first && tz == M && ty == M) continue;
+                run_row(ty, tz, centre_first);
             }
+        } else {
+            run_row(M, M, true);   // centre row first
 #pragma unroll 1
-            for (int ty = 0; ty < E; ++ty)
-                if (!(tz == M && ty == M)) run_row(ty, tz, false);
+            for (int tz = 0; tz < E; ++tz) {
+                if (tz >= 1) refill(tz);
+#pragma unroll 1
+                for (int ty = 0; ty < E; ++ty)
+                    if (!(tz == M && ty == M)) run_row(ty, tz, false);
+            }
         }
         cp_async_wait_all();
 
@@ -392,11 +420,13 @@ cudaError_t launch_pair5_tmr_t(const Dims &dm, const float *f, const float *g, f
 // ---------------------------------------------------------------------------------------------
 // TNLM_VARIANT_PAIRED_TMEM (ref == f): 3^3 patch: whole tile resident at M = 2 (tnlm_pair_tm_kernel), rolling window at
 // M = 3, 4 (tnlm_pair_tmr_kernel); 5^3 patch: rolling window at M = 2, 3, 4 (tnlm_pair5_tmr_kernel).  The 3^3 windows
-// stay on tnlm_pair_kernel / tnlm_pair5_kernel (measured: no gain there).  Where two CTAs per SM are all that fits anyway
-// (3^3 patch at M = 4, 5^3 patch at M = 3) the z-tile is 6 planes deep: a CTA may then take 256 TMEM columns, and the
-// z-halo of the march drops from 6/4 to 8/6 (5^3 patch: 8/4 to 10/6).  +3.6 % and +6.4 % at 128 planes (which 6 does not
-// divide), +4.6 % and +9.7 % at 120.  At M = 4 the 5^3-patch ring does not fit twice at RZ = 6; the three-CTA shapes lose
-// more from the third CTA than the deeper tile gives back (measured, profiles/r02_config5_sweep.md).
+// stay on tnlm_pair_kernel / tnlm_pair5_kernel (measured: no gain there).
+// 3^3 patch at M = 4: only two CTAs per SM fit whatever the depth, so the z-tile is 6 planes deep (a CTA may then take 256
+// TMEM columns; z-halo of the march 8/6 instead of 6/4): +3.6 % at 128 planes (which 6 does not divide), +4.6 % at 120.
+// 5^3 patch: every shape runs TWO CTAs per SM with ~250 registers, which pays for x-offset chunks of 4-5 instead of 2-3
+// (the -ref_i loads, the accumulator round trip and the guard of a pass are spread over twice the offsets) and, where the
+// ring still fits twice (M = 2, 3), for 6-plane tiles (z-halo 10/6 instead of 8/4): 0.427 -> 0.473, 0.415 -> 0.476,
+// 0.429 -> 0.460 of the FP32 roofline at 128 planes (profiles/r02_config5_sweep.md).
 inline bool pair_tm_supported(const tnlm_params &p)
 {
     return (p.patch_radius == 1 || p.patch_radius == 2) && p.search_radius >= 2 && p.search_radius <= 4;
@@ -423,7 +453,7 @@ inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const fl
 {
     if (p.patch_radius == 2) {
         switch (p.search_radius) {
-            case 2: return launch_pair5_tmr_t<2, 4, 3>(dm, f, g, f_out, st);           // <M, RZ, CTAs per SM>
+            case 2: return launch_pair5_tmr_t<2, 6, 2>(dm, f, g, f_out, st);           // <M, RZ, CTAs per SM>
             case 3: return launch_pair5_tmr_t<3, 6, 2>(dm, f, g, f_out, st);           // deep tile: 128 + 128 TMEM columns
             case 4: return launch_pair5_tmr_t<4, 4, 2>(dm, f, g, f_out, st);
             default: return cudaErrorNotSupported;
