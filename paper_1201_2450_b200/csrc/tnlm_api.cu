@@ -577,7 +577,7 @@ int32_t tnlm_z_tile(const tnlm_params *p)
 {
     if (check_params(p) != TNLM_OK) return 0;
     // least common multiple of the tile depths in launch_pair / launch_pair5 / launch_pair_tm (ref == f and separate ref)
-    if (pair_supported(*p)) return p->search_radius >= 3 ? 12 : 4;    // <1,4> <2,4> <3,6> <4,4>; TMEM: 4, 4, 6; SEP: 4, 4, 2, 2
+    if (pair_supported(*p)) return p->search_radius >= 3 ? 12 : 4;    // <1,4> <2,4> <3,6> <4,4>; TMEM: 4, 6, 6; SEP: 4, 4, 2, 2
     if (pair5_supported(*p)) return p->search_radius <= 3 ? 12 : 4;   // 6|4, 4|2, 4|2, 2|2 (ref == f | SEP); TMEM: 6, 6, 4
     return 1;
 }

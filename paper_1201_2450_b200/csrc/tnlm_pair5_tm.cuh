@@ -421,8 +421,8 @@ cudaError_t launch_pair5_tmr_t(const Dims &dm, const float *f, const float *g, f
 // TNLM_VARIANT_PAIRED_TMEM (ref == f): 3^3 patch: whole tile resident at M = 2 (tnlm_pair_tm_kernel), rolling window at
 // M = 3, 4 (tnlm_pair_tmr_kernel); 5^3 patch: rolling window at M = 2, 3, 4 (tnlm_pair5_tmr_kernel).  The 3^3 windows
 // stay on tnlm_pair_kernel / tnlm_pair5_kernel (measured: no gain there).
-// 3^3 patch at M = 4: only two CTAs per SM fit whatever the depth, so the z-tile is 6 planes deep (a CTA may then take 256
-// TMEM columns; z-halo of the march 8/6 instead of 6/4): +3.6 % at 128 planes (which 6 does not divide), +4.6 % at 120.
+// 3^3 patch at M = 3, 4: two CTAs per SM, 6-plane tiles (a CTA may then take 256 TMEM columns; z-halo of the march 8/6
+// instead of 6/4) and all 2M+1 x-offsets of a row in one pass (tnlm_pair_tmr.cuh).
 // 5^3 patch: every shape runs TWO CTAs per SM with ~250 registers, which pays for x-offset chunks of 4-5 instead of 2-3
 // (the -ref_i loads, the accumulator round trip and the guard of a pass are spread over twice the offsets) and, where the
 // ring still fits twice (M = 2, 3), for 6-plane tiles (z-halo 10/6 instead of 8/4): 0.427 -> 0.473, 0.415 -> 0.476,
@@ -461,7 +461,7 @@ inline cudaError_t launch_pair_tm(const tnlm_params &p, const Dims &dm, const fl
     }
     switch (p.search_radius) {
         case 2: return launch_pair_tm_t<2, 4, 16, 3, true>(dm, f, g, f_out, st);   // <M, RZ, TX, CTAs per SM, b in TMEM>
-        case 3: return launch_pair_tmr_t<3, 4, 3>(dm, f, g, f_out, st);            // <M, RZ, CTAs per SM>
+        case 3: return launch_pair_tmr_t<3, 6, 2>(dm, f, g, f_out, st);            // <M, RZ, CTAs per SM>; 256 TMEM columns
         case 4: return launch_pair_tmr_t<4, 6, 2>(dm, f, g, f_out, st);            // deep tile: 256 TMEM columns
         default: return cudaErrorNotSupported;
     }

@@ -10,8 +10,10 @@
 // it is first read.  With the -ref_i windows and (Z, N, b) in TMEM (tnlm_pair_tm.cuh) a CTA needs 69 KB at M = 3,
 // RZ = 4: three CTAs per SM, 12 warps.  Same arithmetic per pass; the ORDER of the passes differs from
 // tnlm_pair_kernel's (centre row, then tz ascending), so results agree with it to rounding, not bit for bit.
-// At M = 4 only two CTAs fit whatever the depth, so the tile is 6 planes deep there (z-halo 8/6 instead of 6/4 on a1 /
-// a2x, 160 TMEM columns per thread out of an allocation of 256): 0.548 -> 0.568 of the FP32 roofline at 128 planes.
+// Two CTAs per SM (NCTA = 2) are a different trade: 6-plane tiles (160 TMEM columns per thread out of an allocation of
+// 256; z-halo of the march 8/6 instead of 6/4) and every x-offset of a row in one pass of 7 or 9 offsets, which ~250
+// registers hold.  Fewer instructions beat the third CTA: 7^3 window 0.543 -> 0.580 of the FP32 roofline at config 4
+// (<3,6,2> against <3,4,3>), 9^3 window 0.549 -> 0.609 (<4,6,2> against <4,4,2> in chunks of 4 + 5).
 #pragma once
 #include "tnlm_pair_tm.cuh"
 
@@ -79,6 +81,10 @@ tnlm_pair_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, f
     using G = PairTmrGeom<M, RZ>;
     using C = Chunks<M>;
     constexpr int TX = 16, NR = G::NR, ACC_W = G::ACC_W, E = G::E;
+    // two CTAs per SM (up to 255 registers) take all 2M+1 x-offsets of a row in ONE pass: the -ref_i loads, the accumulator
+    // round trip through TMEM and the guard are paid once per row instead of once per chunk of 4-5
+    constexpr bool kOneChunk = NCTA == 2;
+    static_assert(!kOneChunk || TX - 2 + 2 * ((E + 4) / 2) <= G::PB2, "a one-chunk row window would leave the tile row");
     constexpr int BP = G::NPB * G::PB2;
     extern __shared__ __align__(16) float smem[];
     float2 *sBE = reinterpret_cast<float2 *>(smem);
@@ -155,8 +161,12 @@ tnlm_pair_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, f
                 if (!frst) fail = pair_pass_tm<RZ, W, false, BP, true, NR>(ta, tacc, row, dm.c2, bexp, 0u, s0);
                 if (__any_sync(0xffffffffu, fail != 0u)) pair_pass_tm<RZ, W, true, BP, true, NR>(ta, tacc, row, dm.c2, bexp, fail, s0);
             };
-            run_chunk(std::integral_constant<int, C::W0>{}, bRow, first);
-            if constexpr (C::W1 > 0) run_chunk(std::integral_constant<int, C::W1>{}, bRow + 4, false);
+            if constexpr (kOneChunk) {
+                run_chunk(std::integral_constant<int, E>{}, bRow, first);
+            } else {
+                run_chunk(std::integral_constant<int, C::W0>{}, bRow, first);
+                if constexpr (C::W1 > 0) run_chunk(std::integral_constant<int, C::W1>{}, bRow + 4, false);
+            }
         };
         // the centre row first: the zero offset is usually the best match, so it sets the reference exponents
         run_row(M, M, true);
