@@ -203,7 +203,6 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
     constexpr int TX = 16, NR = G::NR, E = G::E;
     constexpr bool kZShare = RZ % 2 == 0;   // shared z-sums (pair5_pass_tm) wherever the output planes pair up
     constexpr bool kWide = NCTA == 2;       // two CTAs per SM have the registers for chunks of four or five x-offsets
-    constexpr bool kOneSite = kWide && M == 4;   // three chunk widths: see the pass loop
     extern __shared__ __align__(16) float smem[];
     float2 *sBE = reinterpret_cast<float2 *>(smem);
     float2 *sBO = sBE + G::NPE * G::PB2;
@@ -300,10 +299,9 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
             } else if constexpr (kWide && M == 3) {   // x-offsets 0-3, 4-6
                 run_chunk(std::integral_constant<int, 4>{}, bRow, first_row);
                 run_chunk(std::integral_constant<int, 3>{}, bRow + 4, false);
-            } else if constexpr (kWide && M == 4) {   // x-offsets 4-5, 0-3, 6-8
-                run_chunk(std::integral_constant<int, 2>{}, bRow + 4, first_row);
+            } else if constexpr (kWide && M == 4) {   // x-offsets 4-8 (the zero offset is among them), then 0-3
+                run_chunk(std::integral_constant<int, 5>{}, bRow + 4, first_row);
                 run_chunk(std::integral_constant<int, 4>{}, bRow, false);
-                run_chunk(std::integral_constant<int, 3>{}, bRow + 6, false);
             } else {
 #pragma unroll 1
                 for (int cc = 0; cc < M; ++cc) {
@@ -321,26 +319,13 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
                 stage_plane_async<G>(reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO),
                                      fj + (size_t)clampi(Z0 - 2 - M + pz, dm.Z) * zstride, (tz - 1) % NR, Y0 - 2 - M, X0 - 2 - M, dm, tid);
         };
-        if constexpr (kOneSite) {
-            // one call site for the rows of offsets (with three chunk widths inlined twice each the compiler would
-            // otherwise turn run_row into a function): k = -1 is the centre row, which goes first, then (tz, ty) ascending
+        run_row(M, M, true);   // centre row first
 #pragma unroll 1
-            for (int k = -1; k < E * E; ++k) {
-                const bool centre_first = k < 0;
-                const int tz = centre_first ? M : k / E, ty = centre_first ? M : k - tz * E;
-                if (!centre_first && ty == 0 && tz >= 1) refill(tz);
-                if (!centre_first && tz == M && ty == M) continue;
-                run_row(ty, tz, centre_first);
-            }
-        } else {
-            run_row(M, M, true);   // centre row first
+        for (int tz = 0; tz < E; ++tz) {
+            if (tz >= 1) refill(tz);
 #pragma unroll 1
-            for (int tz = 0; tz < E; ++tz) {
-                if (tz >= 1) refill(tz);
-#pragma unroll 1
-                for (int ty = 0; ty < E; ++ty)
-                    if (!(tz == M && ty == M)) run_row(ty, tz, false);
-            }
+            for (int ty = 0; ty < E; ++ty)
+                if (!(tz == M && ty == M)) run_row(ty, tz, false);
         }
         cp_async_wait_all();
 
@@ -425,8 +410,9 @@ cudaError_t launch_pair5_tmr_t(const Dims &dm, const float *f, const float *g, f
 // instead of 6/4) and all 2M+1 x-offsets of a row in one pass (tnlm_pair_tmr.cuh).
 // 5^3 patch: every shape runs TWO CTAs per SM with ~250 registers, which pays for x-offset chunks of 4-5 instead of 2-3
 // (the -ref_i loads, the accumulator round trip and the guard of a pass are spread over twice the offsets) and, where the
-// ring still fits twice (M = 2, 3), for 6-plane tiles (z-halo 10/6 instead of 8/4): 0.427 -> 0.473, 0.415 -> 0.476,
-// 0.429 -> 0.460 of the FP32 roofline at 128 planes (profiles/r02_config5_sweep.md).
+// ring still fits twice (M = 2, 3), for 6-plane tiles (z-halo 10/6 instead of 8/4): 0.427 -> 0.474, 0.415 -> 0.468,
+// 0.429 -> 0.49 of the FP32 roofline at config 5 (profiles/r02_config5_sweep.md).  Chunks: (5), (4, 3), (5, 4); chunk starts
+// are even so that the LDS.128 of a row window stay aligned.
 inline bool pair_tm_supported(const tnlm_params &p)
 {
     return (p.patch_radius == 1 || p.patch_radius == 2) && p.search_radius >= 2 && p.search_radius <= 4;
