@@ -283,31 +283,46 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
         }
         __syncthreads();
 
-        auto run_row = [&](const int ty, const int tz, const bool first_row) {
+        // one chunk of W x-offsets (starting at x-offset `start`, even) of the row of offsets (ty, tz)
+        auto run_chunk = [&](auto wtag, const int start, const int ty, const int tz, const bool first) {
+            constexpr int W = decltype(wtag)::value;
             const int s0 = tz % NR;
-            const float2 *bRow = ((ty & 1) ? sBO : sBE) + (l + (ty >> 1)) * G::PB2 + x0;
-            auto run_chunk = [&](auto wtag, const float2 *row, const bool first) {
-                constexpr int W = decltype(wtag)::value;
-                unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
-                if (!first) fail = pair5_pass_tm<G, RZ, W, false, kZShare>(t1, t2, row, dm.c2, 0u, s0);
-                if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true, kZShare>(t1, t2, row, dm.c2, fail, s0);
+            const float2 *row = ((ty & 1) ? sBO : sBE) + (l + (ty >> 1)) * G::PB2 + x0 + start;
+            unsigned fail = 0xffffffffu;   // first use: every reference exponent is still +inf
+            if (!first) fail = pair5_pass_tm<G, RZ, W, false, kZShare>(t1, t2, row, dm.c2, 0u, s0);
+            if (__any_sync(0xffffffffu, fail != 0u)) pair5_pass_tm<G, RZ, W, true, kZShare>(t1, t2, row, dm.c2, fail, s0);
+        };
+        // The rows of one tz (tz < 0: the centre row alone, first pass of the direction), CHUNK BY CHUNK: all rows with the
+        // first chunk, then all rows with the second.  Row by row the two unrolled pass bodies (W = 4 and W = 3 at ten planes
+        // each) evict each other from the instruction cache (stall reason no_instruction 0.9 per issued instruction at the
+        // 7^3 window); chunk by chunk each body runs 2M+1 times in a row.  The chunk holding the zero x-offset goes first,
+        // so that the first careful pass sets the reference exponents from the best candidates.
+        auto run_rows = [&](const int tz_or_centre) {
+            const bool centre = tz_or_centre < 0;
+            const int tz = centre ? M : tz_or_centre;
+            auto rows_of = [&](auto wtag, const int start, const bool first_chunk) {
+                if (centre) {
+                    run_chunk(wtag, start, M, M, first_chunk);
+                } else {
+#pragma unroll 1
+                    for (int ty = 0; ty < E; ++ty)
+                        if (!(tz == M && ty == M)) run_chunk(wtag, start, ty, tz, false);
+                }
             };
-            // the chunk holding the zero x-offset (q = M) goes first, so that the first careful pass sets the reference
-            // exponents from the best candidates
             if constexpr (kWide && M == 2) {          // x-offsets 0-4
-                run_chunk(std::integral_constant<int, 5>{}, bRow, first_row);
+                rows_of(std::integral_constant<int, 5>{}, 0, true);
             } else if constexpr (kWide && M == 3) {   // x-offsets 0-3, 4-6
-                run_chunk(std::integral_constant<int, 4>{}, bRow, first_row);
-                run_chunk(std::integral_constant<int, 3>{}, bRow + 4, false);
+                rows_of(std::integral_constant<int, 4>{}, 0, true);
+                rows_of(std::integral_constant<int, 3>{}, 4, false);
             } else if constexpr (kWide && M == 4) {   // x-offsets 4-8 (the zero offset is among them), then 0-3
-                run_chunk(std::integral_constant<int, 5>{}, bRow + 4, first_row);
-                run_chunk(std::integral_constant<int, 4>{}, bRow, false);
-            } else {
+                rows_of(std::integral_constant<int, 5>{}, 4, true);
+                rows_of(std::integral_constant<int, 4>{}, 0, false);
+            } else {                                   // chunks of 2, the last one of 3
 #pragma unroll 1
                 for (int cc = 0; cc < M; ++cc) {
                     const int c = (cc + M / 2) % M;
-                    if (c == M - 1) run_chunk(std::integral_constant<int, 3>{}, bRow + 2 * c, first_row && cc == 0);
-                    else run_chunk(std::integral_constant<int, 2>{}, bRow + 2 * c, first_row && cc == 0);
+                    if (c == M - 1) rows_of(std::integral_constant<int, 3>{}, 2 * c, cc == 0);
+                    else rows_of(std::integral_constant<int, 2>{}, 2 * c, cc == 0);
                 }
             }
         };
@@ -319,13 +334,11 @@ tnlm_pair5_tmr_kernel(const float *__restrict__ f, const float *__restrict__ g, 
                 stage_plane_async<G>(reinterpret_cast<float *>(sBE), reinterpret_cast<float *>(sBO),
                                      fj + (size_t)clampi(Z0 - 2 - M + pz, dm.Z) * zstride, (tz - 1) % NR, Y0 - 2 - M, X0 - 2 - M, dm, tid);
         };
-        run_row(M, M, true);   // centre row first
+        run_rows(-1);   // centre row first
 #pragma unroll 1
         for (int tz = 0; tz < E; ++tz) {
             if (tz >= 1) refill(tz);
-#pragma unroll 1
-            for (int ty = 0; ty < E; ++ty)
-                if (!(tz == M && ty == M)) run_row(ty, tz, false);
+            run_rows(tz);
         }
         cp_async_wait_all();
 
